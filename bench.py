@@ -1,0 +1,369 @@
+#!/usr/bin/env python
+"""bench.py -- Gbonds/s labeled on B200 (BASELINE.json metric), one JSON line on stdout.
+
+A "step" is one pass of the whole hot path -- steps (i)-(iv) of PAPER.md:113 through the public C-ABI call
+ccl_label_bits (ccl_label for the uint8 config 1) -- over one batch of synthetic input: the configured occupancy
+sweep of the workload, one call per p.  Default workload: BASELINE.json config 5 (random 4-regular graph, 2^26
+sites, 2^27 bonds, p in {0.25, 1/3, 0.45}), the configuration north_star's target is quoted on.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1..cfg5] [--impl ours|reference]
+
+N > 1 (under torchrun): independent replicas, one realization per rank, no data-path collective ("replicas only",
+DESIGN.md section "Multi-GPU"); the value is all ranks' bonds over the slowest rank's time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+PC_TR = 0.3473
+WORKLOADS = {
+    # name: (family, size parameter, z, p sweep, mask kind, BASELINE.json config number)
+    "cfg1": ("honeycomb", 64, 0, [0.6527], "u8", 1),
+    "cfg2": ("triangular", 4096, 0, [0.3473], "bits", 2),
+    "cfg3": ("honeycomb", 4096, 0, [0.60, 0.6527, 0.70], "bits", 3),
+    "cfg4": ("regular", 1 << 24, 3, [0.5], "bits", 4),
+    "cfg5": ("regular", 1 << 26, 4, [0.25, 1.0 / 3.0, 0.45], "bits", 5),
+}
+METRIC = "Gbonds/s labeled (1 B200) and achieved HBM GB/s fraction of roofline"
+SEED_BASE = 0x1603083570000000          # DESIGN.md input recipe: seed = SEED_BASE + config number
+CPU_SAMPLE_LOG2_SITES = 22              # cpu_baseline / reference arm: same family at 2^22 sites (bounded sample)
+
+
+def describe(name):
+    fam, size, z, ps, kind, cfg = WORKLOADS[name]
+    if fam == "regular":
+        n, m = size, size * z // 2
+        text = "cfg%d random %d-regular N=2^%d M=%d" % (cfg, z, size.bit_length() - 1, m)
+    else:
+        n = (2 if fam == "honeycomb" else 1) * size * size
+        m = 3 * size * size
+        text = "cfg%d %s L=%d periodic N=%d M=%d" % (cfg, fam, size, n, m)
+    return n, m, text + " p=" + ",".join("%.4g" % p for p in ps) + " mask=" + kind
+
+
+def min_bytes(n, m, kind):
+    """B_min = 8 M (src, dst) + occupancy (M/8 packed, M as uint8) + 12 N (label init write + final
+    read + final write)."""
+    occ = m if kind == "u8" else 4 * ((m + 31) // 32)
+    return 8 * m + occ + 12 * n
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    QUERY = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.QUERY,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            with open(self.path) as f:
+                for line in f:
+                    parts = [t.strip() for t in line.split(",")]
+                    if len(parts) < 6:
+                        continue
+                    try:
+                        sm.append(float(parts[0]))
+                        smax.append(float(parts[1]))
+                    except ValueError:
+                        continue
+                    for nme, val in zip(names, parts[2:6]):
+                        if val.lower().startswith("active"):
+                            reasons.add(nme)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(smax), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def cpu_oracle_sample(name, steps, warmup):
+    """The oracle as it stands, single thread, on a bounded sample of the workload; returns (Gbonds/s, seconds per
+    step, description).  Lattice workloads are sampled at L = 1024, the regular graphs at 2^22 sites."""
+    import numpy as np  # noqa: F401
+    from oracle import oracle
+    fam, size, z, ps, kind, cfg = WORKLOADS[name]
+    seed = SEED_BASE + cfg
+    if fam == "regular":
+        n = min(size, 1 << CPU_SAMPLE_LOG2_SITES)
+        src, dst, _ = oracle.gen_regular(n, z, seed)
+        sample = "random %d-regular graph, N=2^%d sites, M=%d bonds" % (z, n.bit_length() - 1, src.size)
+    else:
+        L = min(size, 1024)
+        src, dst = (oracle.gen_honeycomb if fam == "honeycomb" else oracle.gen_triangular)(L)
+        n = (2 if fam == "honeycomb" else 1) * L * L
+        sample = "%s L=%d, N=%d sites, M=%d bonds" % (fam, L, n, src.size)
+    masks = [oracle.gen_occupancy(src.size, p, seed, 0) for p in ps]
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        for mask, bits in masks:
+            if kind == "u8":
+                oracle.label(n, src, dst, mask)
+            else:
+                oracle.label_bits(n, src, dst, bits)
+        if it >= warmup:
+            times.append(time.perf_counter() - t0)
+    per_step = sum(times) / len(times)
+    sample += ", p sweep " + ",".join("%.4g" % p for p in ps) + ", same seeds; labeling time only (oracle_label%s)" % (
+        "" if kind == "u8" else "_bits")
+    return len(ps) * src.size / per_step / 1e9, per_step, sample
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores (this tier has no other reference implementation)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n, m, text = describe(args.workload)
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    # keep the whole run within a few minutes: a 2^22-site sweep costs about 2 s per step
+    steps_eff, warmup_eff = min(steps, 20), min(warmup, 3)
+    value, per_step, sample = cpu_oracle_sample(args.workload, steps_eff, warmup_eff)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "Gbonds/s", "n_gpus": args.gpus,
+        "steps": steps_eff, "warmup": warmup_eff, "ms_per_step": per_step * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": {"workload": text, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "Gbonds/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "Gbonds/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1603_08357_b200 as ccl      # raises if libccl.so cannot be built/loaded: no fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    fam, size, z, ps, kind, cfg = WORKLOADS[args.workload]
+    n, m, text = describe(args.workload)
+    seed = SEED_BASE + cfg
+    # ---- synthetic inputs, generated on the device by the library's own seeded generators (untimed)
+    if fam == "regular":
+        src, dst = ccl.gen_regular(n, z, seed)
+    elif fam == "honeycomb":
+        src, dst = ccl.gen_honeycomb(size)
+    else:
+        src, dst = ccl.gen_triangular(size)
+    masks = []
+    for p in ps:                      # replicas differ by realization = rank
+        mask, bits = ccl.gen_occupancy(m, p, seed, rank, want_mask=(kind == "u8"), want_bits=(kind != "u8"))
+        masks.append(mask if kind == "u8" else bits)
+    labels = torch.empty(n, dtype=torch.int32, device="cuda")
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+
+    def one_call(k):
+        if kind == "u8":
+            ccl.label(n, src, dst, masks[k], labels=labels)
+        else:
+            ccl.label_bits(n, src, dst, masks[k], labels=labels)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # L2 hygiene: the bond stream of cfg2-5 (0.2-1.1 GB) exceeds the 126 MB L2, so every call streams from HBM; for
+    # the small cfg1 an L2-sized buffer is rewritten between timed calls.
+    flush = None
+    if min_bytes(n, m, kind) < 512 * 1024 * 1024:
+        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+
+    for _ in range(max(3, args.warmup)):
+        for k in range(len(ps)):
+            one_call(k)
+    barrier()
+
+    K = max(1, args.steps)
+    ncalls = K * len(ps)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(ncalls)]
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches0 = ccl.launch_count()
+    barrier()
+    t_start = torch.cuda.Event(enable_timing=True)
+    t_stop = torch.cuda.Event(enable_timing=True)
+    flush_ms = 0.0
+    t_start.record()
+    c = 0
+    for _ in range(K):
+        for k in range(len(ps)):
+            if flush is not None:
+                flush.fill_(c & 0xFF)
+            e = ev[c]
+            ccl.set_profile_events(e[1], e[2], e[3])
+            e[0].record()
+            one_call(k)
+            c += 1
+    t_stop.record()
+    barrier()
+    launches = ccl.launch_count() - launches0
+    clocks = sampler.stop()
+    ccl.set_profile_events(None, None, None)
+    total_ms = t_start.elapsed_time(t_stop)
+    call_ms = [e[0].elapsed_time(e[3]) for e in ev]
+    init_ms = [e[0].elapsed_time(e[1]) for e in ev]
+    reduce_ms = [e[1].elapsed_time(e[2]) for e in ev]
+    flat_ms = [e[2].elapsed_time(e[3]) for e in ev]
+    if flush is not None:
+        total_ms = sum(call_ms)                       # exclude the flush writes from the step time
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / K
+    value = world * len(ps) * m / (ms_per_step * 1e-3) / 1e9
+
+    peak, peak_src = measured_peak()
+    avg = lambda xs: sum(xs) / len(xs)
+    stream_bytes = 8 * m + (m if kind == "u8" else 4 * ((m + 31) // 32))
+    ach = stream_bytes / (avg(reduce_ms) * 1e-3) / 1e9
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get(args.workload, {}).get("k_reduce_dram_bytes_per_launch")
+    except Exception:
+        pass
+    call_ach = min_bytes(n, m, kind) / (avg(call_ms) * 1e-3) / 1e9
+    per_p = {}
+    for k, p in enumerate(ps):
+        sel = [i for i in range(ncalls) if i % len(ps) == k]
+        t = avg([call_ms[i] for i in sel])
+        per_p["%.4g" % p] = {"ms": t, "init_ms": avg([init_ms[i] for i in sel]),
+                             "reduce_ms": avg([reduce_ms[i] for i in sel]), "flatten_ms": avg([flat_ms[i] for i in sel]),
+                             "gbonds_per_s": m / (t * 1e-3) / 1e9, "gsites_per_s": n / (t * 1e-3) / 1e9,
+                             "roofline_frac_measured": min_bytes(n, m, kind) / (t * 1e-3) / 1e9 / peak,
+                             "roofline_frac_8TBs": min_bytes(n, m, kind) / (t * 1e-3) / 1e9 / 8000.0}
+
+    # ---- end to end through the host-buffer entry point: H2D of the inputs and D2H of the labels inside the timing
+    e2e = None
+    if not args.no_e2e and kind != "u8":
+        hs, hd = src.cpu().pin_memory(), dst.cpu().pin_memory()
+        hm = [b.cpu().pin_memory() for b in masks]
+        hl = torch.empty(n, dtype=torch.int32).pin_memory()
+        ccl.label_bits_host(n, hs, hd, hm[0], hl)                     # warm-up (memory pool, page tables)
+        e2e_steps = max(1, min(K, 3))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            for k in range(len(ps)):
+                ccl.label_bits_host(n, hs, hd, hm[k], hl)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        h2d = len(ps) * (2 * 4 * m + 4 * ((m + 31) // 32))
+        d2h = len(ps) * 4 * n
+        e2e = {"value": world * len(ps) * m * e2e_steps / dt / 1e9, "unit": "Gbonds/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+               "api": "ccl_label_bits_host (pinned host src/dst/bits in, host labels out, synchronous)"}
+        del hs, hd, hm, hl
+
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        v, per_step, sample = cpu_oracle_sample(args.workload, 3, 1)
+        cpu = {"value": v, "unit": "Gbonds/s", "cores": 1, "kind": "oracle", "sample": sample,
+               "host_cores_available": os.cpu_count()}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "Gbonds/s", "n_gpus": world, "steps": K,
+            "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": text, "calls_per_step": len(ps), "api": "ccl_label" if kind == "u8" else "ccl_label_bits",
+                       "parallelism": "replicas x%d (one realization per GPU, no collective)" % world,
+                       "l2": "inputs larger than L2 (bond stream %.0f MB per call vs 126 MB L2)" % (stream_bytes / 1e6)
+                       if flush is None else "256 MB buffer rewritten between timed calls (L2 flush)",
+                       "gsites_per_s": world * len(ps) * n / (ms_per_step * 1e-3) / 1e9},
+            "roofline": {"bound": "hbm", "kernel": "k_reduce (step iii)", "achieved": ach, "peak": peak, "unit": "GB/s",
+                         "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": stream_bytes, "avg_launch_ms": avg(reduce_ms),
+                         "share_of_call": avg(reduce_ms) / avg(call_ms)},
+            "roofline_call": {"bound": "hbm", "what": "whole ccl_label call, B_min = 8M + mask + 12N (SURVEY 8(d))",
+                              "achieved": call_ach, "peak": peak, "unit": "GB/s", "frac": call_ach / peak,
+                              "frac_of_8TBs_nominal": call_ach / 8000.0, "bytes_per_call": min_bytes(n, m, kind),
+                              "avg_call_ms": avg(call_ms)},
+            "per_p": per_p, "kernel_ms": {"k_init": avg(init_ms), "k_reduce": avg(reduce_ms), "k_flatten": avg(flat_ms)},
+            "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,131 @@
+/*
+ * ccl.h -- C ABI of libccl.so: bond-list connected-component labeling for sm_100a (NVIDIA B200).
+ *
+ * The operation is the hot path of Y. Komura, "A generalized GPU-based connected component labeling
+ * algorithm" (arXiv 1603.08357; PAPER.md), section 3: four steps -- (i) initialization, (ii) analysis,
+ * (iii) label reduction with atomicMin (Algorithm 1), (iv) analysis --
+ * with the nearest-neighbour list of PAPER.md:111 replaced by a bond list plus per-bond occupancy
+ * (BASELINE.json north_star).  The result is the canonical labeling of PAPER.md:115:
+ *
+ *        labels[i] = smallest site index in the connected component of site i.
+ *
+ * Conventions for every entry point
+ *   - All array pointers are DEVICE pointers owned by the caller unless the name says `host_`.  The library
+ *     never frees caller memory and keeps no allocation alive after a call returns.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the default stream).  All work is enqueued on it; no
+ *     entry point synchronises with the host unless stated.  Results are valid once the stream has drained.
+ *   - Return value: CCL_OK (0) or a ccl_status.  No exception crosses the ABI.  ccl_last_error() returns a
+ *     thread-local, NUL-terminated description of the last failure on the calling thread.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns CCL_CUDA_ERROR.
+ */
+#ifndef CCL_H_
+#define CCL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum ccl_status {
+    CCL_OK = 0,
+    CCL_INVALID_ARG = 1,          /* negative count, count > 2^31-1 sites, NULL where data is required */
+    CCL_CUDA_ERROR = 2,           /* a CUDA runtime call or launch failed; see ccl_last_error()         */
+    CCL_UNSUPPORTED = 3,          /* argument combination the library does not implement               */
+    CCL_WORKSPACE_TOO_SMALL = 4   /* caller-provided workspace is smaller than the size query reported  */
+} ccl_status;
+
+/* Result of ccl_cluster_stats (reading R8).  Lives in device memory; 32 bytes. */
+typedef struct ccl_stats {
+    int64_t  n_clusters;      /* #{ i : labels[i] == i }                                             */
+    int64_t  largest;         /* size of the largest cluster                                          */
+    int64_t  largest_label;   /* its label; ties broken towards the smallest label                    */
+    uint64_t sum_s2;          /* sum over clusters of size^2 (<= N^2 < 2^63 for N <= 2^31)             */
+} ccl_stats;
+
+/* ---- the hot path: steps (i)-(iv), PAPER.md:113 ------------------------------------------------------
+ *
+ * ccl_label: bonds b = 0..n_bonds-1 join sites src[b] and dst[b] (two separate int32 arrays); bond b is
+ * occupied iff occupied[b] != 0 (one uint8 per bond); occupied == NULL means every bond is occupied.
+ * labels[n_sites] (int32) is write-only on entry -- no initial content is required -- and holds the canonical
+ * labels on completion.  src, dst, occupied are read-only.  0 <= src[b], dst[b] < n_sites is a caller
+ * precondition that is NOT checked here (use ccl_validate_bonds).  Self-loops and repeated bonds are legal.
+ * n_bonds == 0 gives labels[i] = i.  n_sites == 0 is a no-op.  The result does not depend on bond order.
+ * Errors: n_sites < 0, n_sites > 2^31-1, n_bonds < 0, or NULL src/dst/labels with a non-zero count
+ * -> CCL_INVALID_ARG.
+ */
+int ccl_label(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+              const uint8_t* occupied, int32_t* labels, void* stream);
+
+/* Same with a packed mask: bond b is bit (b & 31) of uint32 word (b >> 5); ceil(n_bonds/32) words, bits past
+ * n_bonds are ignored.  src and dst should be 16-byte aligned for the vectorised path (any alignment works). */
+int ccl_label_bits(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+                   const uint32_t* occupied_bits, int32_t* labels, void* stream);
+
+/* Debug validator: *out_bad (device int64) = number of bonds with an endpoint outside [0, n_sites). */
+int ccl_validate_bonds(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+                       int64_t* out_bad, void* stream);
+
+/* ---- seeded workload generators (outside the timed metric) -----------------
+ *
+ * Periodic L x L lattices, 3*L*L bonds each (the paper names the lattices only; geometry and
+ * numbering are this project's, reading R9):
+ *   triangular: site s = y*L + x; bond 3s+k joins s to (x+1,y), (x,y+1), (x+1,y+1) mod L for k = 0,1,2.
+ *   honeycomb : cell c = y*L + x holds sites A = 2c, B = 2c+1; bond 3c+0 = A(c)-B(c), 3c+1 = B(c)-A(x+1,y),
+ *               3c+2 = B(c)-A(x,y+1) mod L; src is the first-named site.
+ * L >= 1 and 2*L*L <= 2^31-1.
+ */
+int ccl_gen_triangular(int32_t L, int32_t* src, int32_t* dst, void* stream);
+int ccl_gen_honeycomb(int32_t L, int32_t* src, int32_t* dst, void* stream);
+
+/* Simple random z-regular graph on n_sites sites by the configuration model ("Bethe substitute" of
+ * BASELINE.json configs 4-5; the paper's own Bethe workload is the Cayley tree):
+ * n_sites*z/2 bonds in uniformly random order; stub keys from Philox4x32-10, stable sort, defects (self-loops,
+ * repeated pairs) repaired by seeded endpoint swaps.  Call with workspace == NULL to obtain the required size in
+ * *workspace_bytes (host pointer); then call again with a device workspace of at least that size.
+ * n_sites*z must be even, 1 <= z <= 16, n_sites*z <= 2^31-1. */
+int ccl_gen_regular(int64_t n_sites, int32_t z, uint64_t seed, int32_t* src, int32_t* dst,
+                    void* workspace, size_t* workspace_bytes, void* stream);
+
+/* Bernoulli(p) occupancy: T = floor(p*2^32) computed on the host in double; bond b is occupied iff word (b & 3)
+ * of Philox4x32-10(counter = (b>>2 lo, b>>2 hi, realization, 0), key = (seed lo, seed hi)) < T; p >= 1 occupies
+ * everything.  Writes whichever of the two outputs is non-NULL: a uint8 0/1 mask [n_bonds] and/or packed bits
+ * [ceil(n_bonds/32) words, unused high bits zero].  The same seed at two values of p gives nested sets. */
+int ccl_gen_occupancy(int64_t n_bonds, double p, uint64_t seed, uint32_t realization,
+                      uint8_t* mask_or_null, uint32_t* bits_or_null, void* stream);
+
+/* ---- cluster statistics from canonical labels (outside the timed metric) -----------------------------
+ *
+ * size_scratch: device int32[n_sites], overwritten (cluster sizes indexed by label).  out: device ccl_stats.
+ * hist_dense (optional): device int64[n_dense+1]; hist_dense[s] = number of clusters of size exactly s,
+ * 1 <= s <= n_dense; entry 0 is set to 0.  hist_log2 (optional): device int64[32]; hist_log2[k] = number of
+ * clusters with 2^k <= size < 2^(k+1).  labels must be canonical (output of ccl_label*). */
+int ccl_cluster_stats(int64_t n_sites, const int32_t* labels, int32_t* size_scratch, ccl_stats* out,
+                      int64_t* hist_dense, int32_t n_dense, int64_t* hist_log2, void* stream);
+
+/* ---- whole-call convenience with HOST buffers (the end-to-end path bench.py times as "e2e") ----------
+ *
+ * Copies src/dst/occupied_bits from host memory (pinned for full speed) to device scratch the call allocates and
+ * frees, runs ccl_label_bits, copies labels back to host_labels and synchronises the stream before returning. */
+int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_src, const int32_t* host_dst,
+                        const uint32_t* host_occupied_bits, int32_t* host_labels, void* stream);
+
+/* ---- profiling hook ------------------------------------------------------------------------------------
+ *
+ * Optional cudaEvent_t handles (as void*, any of them NULL = off) that the NEXT ccl_label / ccl_label_bits calls on
+ * this host thread record on their stream: after step (i) (k_init), after step (iii) (k_reduce) and after step
+ * (iv) (k_flatten).  Together with an event the caller records before the call they give each step's device time
+ * from inside the caller's own timed region.  The handles stay in force until replaced; pass three NULLs to clear. */
+int ccl_set_profile_events(void* after_init, void* after_reduce, void* after_flatten);
+
+/* ---- diagnostics ------------------------------------------------------------------------------------- */
+const char* ccl_last_error(void);      /* thread-local; never NULL                                      */
+int ccl_version(void);                 /* 10000*major + 100*minor + patch                                */
+/* Number of kernels this library has launched on the calling thread since load (bench.py's gpu_launches). */
+int64_t ccl_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CCL_H_ */

@@ -1,0 +1,184 @@
+"""ctypes binding of libccl.so.  Same names as include/ccl.h without the `ccl_` prefix; marshalling only.
+
+Every compute call takes torch CUDA tensors (device memory owned by the caller) and enqueues on torch's current
+stream.  Nothing here computes: every step of the path runs in the CUDA kernels of csrc/.
+"""
+import ctypes as C
+
+import torch
+
+from .build import build
+
+_LIB_PATH = build()            # raises if nvcc fails: no fallback
+lib = C.CDLL(_LIB_PATH)
+
+EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangular", "ccl_gen_honeycomb",
+           "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
+           "ccl_set_profile_events", "ccl_last_error",
+           "ccl_version", "ccl_launch_count"]
+
+_vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
+lib.ccl_label.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp]
+lib.ccl_label_bits.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp]
+lib.ccl_label_bits_host.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp]
+lib.ccl_validate_bonds.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp]
+lib.ccl_gen_triangular.argtypes = [_i32, _vp, _vp, _vp]
+lib.ccl_gen_honeycomb.argtypes = [_i32, _vp, _vp, _vp]
+lib.ccl_gen_regular.argtypes = [_i64, _i32, _u64, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
+lib.ccl_gen_occupancy.argtypes = [_i64, C.c_double, _u64, _u32, _vp, _vp, _vp]
+lib.ccl_cluster_stats.argtypes = [_i64, _vp, _vp, _vp, _vp, _i32, _vp, _vp]
+lib.ccl_last_error.restype = C.c_char_p
+lib.ccl_last_error.argtypes = []
+lib.ccl_version.argtypes = []
+lib.ccl_launch_count.restype = _i64
+lib.ccl_launch_count.argtypes = []
+lib.ccl_set_profile_events.argtypes = [_vp, _vp, _vp]
+for _n in EXPORTS[:10]:
+    getattr(lib, _n).restype = C.c_int
+
+
+class CclError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = code
+        super().__init__("%s failed with status %d: %s" % (what, code, last_error()))
+
+
+def last_error():
+    return lib.ccl_last_error().decode()
+
+
+def version():
+    return lib.ccl_version()
+
+
+def launch_count():
+    return int(lib.ccl_launch_count())
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise CclError(rc, what)
+
+
+def _stream():
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _dev(t, dtype, what):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError("%s must be a contiguous CUDA tensor of dtype %s" % (what, dtype))
+    return t.data_ptr()
+
+
+def label(n_sites, src, dst, occupied=None, labels=None):
+    """ccl_label: uint8 mask (or None = all bonds occupied).  Returns the int32 label tensor."""
+    if labels is None:
+        labels = torch.empty(n_sites, dtype=torch.int32, device=src.device)
+    _check(lib.ccl_label(n_sites, src.numel(), _dev(src, torch.int32, "src"), _dev(dst, torch.int32, "dst"),
+                         _dev(occupied, torch.uint8, "occupied"), _dev(labels, torch.int32, "labels"), _stream()),
+           "ccl_label")
+    return labels
+
+
+def label_bits(n_sites, src, dst, occupied_bits, labels=None, n_bonds=None):
+    """ccl_label_bits: packed mask as an int32 tensor of ceil(n_bonds/32) words (bit b&31 of word b>>5)."""
+    if labels is None:
+        labels = torch.empty(n_sites, dtype=torch.int32, device=src.device)
+    m = src.numel() if n_bonds is None else n_bonds
+    _check(lib.ccl_label_bits(n_sites, m, _dev(src, torch.int32, "src"), _dev(dst, torch.int32, "dst"),
+                              _dev(occupied_bits, torch.int32, "occupied_bits"),
+                              _dev(labels, torch.int32, "labels"), _stream()), "ccl_label_bits")
+    return labels
+
+
+def _host(t, what):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()):
+        raise TypeError("%s must be a contiguous CPU int32 tensor" % what)
+    return t.data_ptr()
+
+
+def label_bits_host(n_sites, src, dst, occupied_bits, labels):
+    """ccl_label_bits_host: HOST tensors in (pinned for full speed), host labels out; synchronises."""
+    _check(lib.ccl_label_bits_host(n_sites, src.numel(), _host(src, "src"), _host(dst, "dst"),
+                                   _host(occupied_bits, "occupied_bits"), _host(labels, "labels"), _stream()),
+           "ccl_label_bits_host")
+    return labels
+
+
+def set_profile_events(after_init=None, after_reduce=None, after_flatten=None):
+    """ccl_set_profile_events with torch.cuda.Event objects (created with enable_timing=True) or None."""
+    def h(e):
+        if e is None:
+            return None
+        e.record()                      # torch creates the underlying cudaEvent_t lazily: force it into existence
+        return e.cuda_event
+    _check(lib.ccl_set_profile_events(h(after_init), h(after_reduce), h(after_flatten)), "ccl_set_profile_events")
+
+
+def validate_bonds(n_sites, src, dst):
+    """Number of bonds with an endpoint outside [0, n_sites) (synchronises to return a Python int)."""
+    out = torch.zeros(1, dtype=torch.int64, device=src.device)
+    _check(lib.ccl_validate_bonds(n_sites, src.numel(), _dev(src, torch.int32, "src"), _dev(dst, torch.int32, "dst"),
+                                  out.data_ptr(), _stream()), "ccl_validate_bonds")
+    return int(out.item())
+
+
+def _lattice(fn, name, L, device):
+    m = 3 * L * L
+    src = torch.empty(m, dtype=torch.int32, device=device)
+    dst = torch.empty(m, dtype=torch.int32, device=device)
+    _check(fn(L, src.data_ptr(), dst.data_ptr(), _stream()), name)
+    return src, dst
+
+
+def gen_triangular(L, device="cuda"):
+    return _lattice(lib.ccl_gen_triangular, "ccl_gen_triangular", L, device)
+
+
+def gen_honeycomb(L, device="cuda"):
+    return _lattice(lib.ccl_gen_honeycomb, "ccl_gen_honeycomb", L, device)
+
+
+def gen_regular(n_sites, z, seed, device="cuda"):
+    m = n_sites * z // 2
+    need = C.c_size_t(0)
+    _check(lib.ccl_gen_regular(n_sites, z, seed, None, None, None, C.byref(need), _stream()), "ccl_gen_regular(size)")
+    ws = torch.empty(need.value, dtype=torch.uint8, device=device)
+    src = torch.empty(m, dtype=torch.int32, device=device)
+    dst = torch.empty(m, dtype=torch.int32, device=device)
+    _check(lib.ccl_gen_regular(n_sites, z, seed, src.data_ptr(), dst.data_ptr(), ws.data_ptr(), C.byref(need),
+                               _stream()), "ccl_gen_regular")
+    del ws
+    return src, dst
+
+
+def gen_occupancy(n_bonds, p, seed, realization=0, want_mask=True, want_bits=True, device="cuda"):
+    """(uint8 mask or None, int32-typed packed bits or None)."""
+    mask = torch.empty(n_bonds, dtype=torch.uint8, device=device) if want_mask else None
+    bits = torch.empty((n_bonds + 31) // 32, dtype=torch.int32, device=device) if want_bits else None
+    _check(lib.ccl_gen_occupancy(n_bonds, float(p), seed, realization, None if mask is None else mask.data_ptr(),
+                                 None if bits is None else bits.data_ptr(), _stream()), "ccl_gen_occupancy")
+    return mask, bits
+
+
+class Stats(C.Structure):
+    _fields_ = [("n_clusters", C.c_int64), ("largest", C.c_int64), ("largest_label", C.c_int64), ("sum_s2", C.c_uint64)]
+
+
+def cluster_stats(labels, n_dense=0):
+    """(dict of exact integers, hist_dense[n_dense+1] int64 CPU tensor, hist_log2[32]); synchronises to read back."""
+    n = labels.numel()
+    dev = labels.device
+    scratch = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    out = torch.empty(4, dtype=torch.int64, device=dev)
+    hd = torch.empty(n_dense + 1, dtype=torch.int64, device=dev)
+    hl = torch.empty(32, dtype=torch.int64, device=dev)
+    _check(lib.ccl_cluster_stats(n, _dev(labels, torch.int32, "labels"), scratch.data_ptr(), out.data_ptr(),
+                                 hd.data_ptr(), n_dense, hl.data_ptr(), _stream()), "ccl_cluster_stats")
+    o = out.cpu().tolist()
+    d = dict(n_clusters=o[0], largest=o[1], largest_label=o[2], sum_s2=o[3] & 0xFFFFFFFFFFFFFFFF)
+    return d, hd.cpu(), hl.cpu()

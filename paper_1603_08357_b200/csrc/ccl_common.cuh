@@ -1,0 +1,99 @@
+// ccl_common.cuh -- host-side plumbing shared by the translation units of libccl.so (error string, launch
+// counter, stream cast) and the small device helpers (cache-hinted loads/stores).  Product code: nothing under
+// oracle/ is included from here or includes this.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/ccl.h"
+
+namespace ccl {
+
+constexpr int kSMs = 148;                 // B200: 2 dies x 74 SMs
+
+// ---- host plumbing ---------------------------------------------------------------------------------------
+void set_error(const char* fmt, ...);
+void count_launch(int n = 1);
+
+inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s); }
+
+#define CCL_CUDA_TRY(expr)                                                                         \
+    do {                                                                                           \
+        cudaError_t err__ = (expr);                                                                \
+        if (err__ != cudaSuccess) {                                                                \
+            ::ccl::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(err__), __FILE__,   \
+                             __LINE__);                                                            \
+            return CCL_CUDA_ERROR;                                                                 \
+        }                                                                                          \
+    } while (0)
+
+#define CCL_CHECK_LAUNCH(name)                                                                     \
+    do {                                                                                           \
+        cudaError_t err__ = cudaGetLastError();                                                    \
+        if (err__ != cudaSuccess) {                                                                \
+            ::ccl::set_error("launch of %s failed: %s", name, cudaGetErrorString(err__));          \
+            return CCL_CUDA_ERROR;                                                                 \
+        }                                                                                          \
+        ::ccl::count_launch();                                                                     \
+    } while (0)
+
+#define CCL_REQUIRE(cond, msg)                                                                     \
+    do {                                                                                           \
+        if (!(cond)) {                                                                             \
+            ::ccl::set_error("invalid argument: %s", msg);                                         \
+            return CCL_INVALID_ARG;                                                                \
+        }                                                                                          \
+    } while (0)
+
+// ---- device helpers --------------------------------------------------------------------------------------
+// Streaming (read-once) loads: bypass L1 allocation and mark the L2 line evict-first, so that the bond stream
+// does not push label[] sectors out of L2.
+__device__ __forceinline__ uint64_t evict_first_policy()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ int4 ld_stream_v4(const int32_t* p, uint64_t pol)
+{
+    int4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.s32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ int32_t ld_stream_s32(const int32_t* p, uint64_t pol)
+{
+    int32_t r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.s32 %0, [%1], %2;" : "=r"(r) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_stream_u32(const uint32_t* p, uint64_t pol)
+{
+    uint32_t r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.u32 %0, [%1], %2;" : "=r"(r) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_stream_u8(const uint8_t* p, uint64_t pol)
+{
+    uint32_t r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.u8 %0, [%1], %2;" : "=r"(r) : "l"(p), "l"(pol));
+    return r;
+}
+
+// Label reads during root finding.  Relaxed, L2-coherent (bypasses the non-coherent L1): a stale value would
+// still be a valid ancestor, but fresh values shorten the walks.
+__device__ __forceinline__ int32_t ld_label(const int32_t* p)
+{
+    int32_t r;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(r) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st_label(int32_t* p, int32_t v)
+{
+    asm volatile("st.relaxed.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+}  // namespace ccl

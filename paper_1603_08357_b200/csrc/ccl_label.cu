@@ -1,0 +1,321 @@
+// ccl_label.cu -- steps (i)-(iv) of Komura's generalized CCL on a bond list, for sm_100a.
+//
+//   k_init     step (i)   label[i] = i                       (BASELINE.json north_star form; with it step (ii),
+//                         the first analysis, has nothing to do: every site is its own root -- DESIGN.md R1)
+//   k_reduce   step (iii) one pass over the bond stream; every occupied bond runs Algorithm 1
+//                         (PAPER.md:118-149): atomicMin(&label[larger], smaller), following the returned value
+//   k_flatten  step (iv)  label[i] <- root(i)                ("analysis", Fig. 4)
+//
+// Everything is integer work on int32 labels; the bound is HBM / L2 gather traffic, so there are no tensor cores
+// here.
+#include "ccl_common.cuh"
+
+namespace ccl {
+
+constexpr int kThreads = 256;
+
+// ------------------------------------------------------------------------------------------------ step (i)
+__global__ void __launch_bounds__(kThreads) k_init(int64_t n_sites, int32_t* __restrict__ label)
+{
+    const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
+    for (int64_t i = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; i < n_sites; i += stride) {
+        if (i + 4 <= n_sites) {
+            const int32_t b = (int32_t)i;
+            *reinterpret_cast<int4*>(label + i) = make_int4(b, b + 1, b + 2, b + 3);   // label is 16 B aligned
+        } else {
+            for (int64_t j = i; j < n_sites; ++j) label[j] = (int32_t)j;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ root finding
+// Walk label[label[...]] to the root, halving the path on the way: every visited site is
+// re-pointed at its grandparent.  A shortcut store can only write an ancestor, so it never disconnects anything
+// (DESIGN.md "Concurrency").
+__device__ __forceinline__ int32_t find_root(int32_t* label, int32_t x)
+{
+    int32_t p = ld_label(label + x);
+    while (p != x) {
+        const int32_t gp = ld_label(label + p);
+        if (gp == p) return p;
+        st_label(label + x, gp);
+        x = gp;
+        p = ld_label(label + x);
+    }
+    return x;
+}
+
+// Algorithm 1 (reading R3 of its garbled last lines, exit test R4): make sure sites a and b end
+// up in one tree.  label_1 is the larger of the two current representatives, label_2 the smaller.
+__device__ __forceinline__ void algorithm1(int32_t* label, int32_t a, int32_t b)
+{
+    int32_t label_1 = find_root(label, a);
+    int32_t label_2 = find_root(label, b);
+    while (label_1 != label_2) {
+        if (label_1 < label_2) { const int32_t t = label_1; label_1 = label_2; label_2 = t; }
+        const int32_t label_3 = atomicMin(label + label_1, label_2);
+        if (label_3 == label_1 || label_3 == label_2) return;     // linked now / was linked already
+        // label_1 was not a root any more.  If label_3 > label_2 the link label_1 -> label_3 has just been
+        // replaced by label_1 -> label_2, so label_3 must be joined to label_2; if label_3 < label_2 nothing was
+        // written and label_1 hangs under label_3, which must be joined to label_2.  Either way the pair to join
+        // is (label_3, label_2); walk both up to their roots before the next atomic.
+        label_1 = find_root(label, label_3);
+        label_2 = find_root(label, label_2);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------- step (iii)
+// MASK: 0 = every bond occupied, 1 = uint8 per bond, 2 = packed bits.  VEC: src/dst 16-byte aligned (and the
+// uint8 mask 4-byte aligned), so a thread fetches its 4 bonds with two 128-bit loads.
+template <int MASK, bool VEC>
+__global__ void __launch_bounds__(kThreads)
+k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
+         const void* __restrict__ occ, int32_t* label)
+{
+    const int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
+    if (b0 >= n_bonds) return;
+    const int cnt = (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
+    const uint64_t pol = evict_first_policy();
+
+    // occupancy of this thread's 4 bonds -> low 4 bits of m
+    uint32_t m = 0xFu;
+    if (MASK == 2) {
+        m = (ld_stream_u32(static_cast<const uint32_t*>(occ) + (b0 >> 5), pol) >> (b0 & 31)) & 0xFu;   // b0 % 4 == 0
+    } else if (MASK == 1) {
+        const uint8_t* o = static_cast<const uint8_t*>(occ) + b0;
+        if (VEC && cnt == 4) {
+            const uint32_t w = ld_stream_u32(reinterpret_cast<const uint32_t*>(o), pol);
+            m = ((w & 0xFFu) != 0) | (((w & 0xFF00u) != 0) << 1) | (((w & 0xFF0000u) != 0) << 2) |
+                (((w & 0xFF000000u) != 0) << 3);
+        } else {
+            m = 0;
+            for (int k = 0; k < cnt; ++k) m |= (uint32_t)(ld_stream_u8(o + k, pol) != 0) << k;
+        }
+    }
+    m &= (1u << cnt) - 1u;
+    if (m == 0) return;
+
+    int32_t u[4], v[4];
+    if (VEC && cnt == 4) {
+        const int4 s = ld_stream_v4(src + b0, pol), d = ld_stream_v4(dst + b0, pol);
+        u[0] = s.x; u[1] = s.y; u[2] = s.z; u[3] = s.w;
+        v[0] = d.x; v[1] = d.y; v[2] = d.z; v[3] = d.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            u[k] = (k < cnt) ? ld_stream_s32(src + b0 + k, pol) : 0;
+            v[k] = (k < cnt) ? ld_stream_s32(dst + b0 + k, pol) : 0;
+        }
+    }
+
+    // First touch: Algorithm 1's atomicMin applied straight to the bond's own endpoints, all four in flight at
+    // once.  If the higher site was still a root this IS the link (the paper's step (i) hook, done
+    // as the first wave of step (iii)); otherwise the returned value tells which pair is left to join.
+    int32_t lo[4], old[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        lo[k] = min(u[k], v[k]);
+        const int32_t hi = max(u[k], v[k]);
+        old[k] = lo[k];                                    // "nothing left to do"
+        if (((m >> k) & 1u) && hi != lo[k]) {
+            const int32_t o = atomicMin(label + hi, lo[k]);
+            old[k] = (o == hi) ? lo[k] : o;
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (old[k] != lo[k]) algorithm1(label, old[k], lo[k]);
+}
+
+// ----------------------------------------------------------------------------------------------- step (iv)
+// Every site follows its chain to the root and stores it (reading R2: per-site chase).  Concurrent
+// writers only ever replace a chain pointer by the root of the same chain, so a reader sees either and still
+// arrives at the root.  Roots and already-flat sites are not rewritten.
+__global__ void __launch_bounds__(kThreads) k_flatten(int64_t n_sites, int32_t* label)
+{
+    const int64_t i0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
+    if (i0 >= n_sites) return;
+    if (i0 + 4 <= n_sites) {
+        int4 l = *reinterpret_cast<const int4*>(label + i0);
+        int32_t cur[4] = {l.x, l.y, l.z, l.w};
+        int32_t par[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) par[k] = (cur[k] == (int32_t)(i0 + k)) ? cur[k] : ld_label(label + cur[k]);
+        bool changed = false;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            int32_t c = cur[k], p = par[k];
+            while (p != c) { c = p; p = ld_label(label + c); }
+            changed |= (c != cur[k]);
+            cur[k] = c;
+        }
+        if (changed) *reinterpret_cast<int4*>(label + i0) = make_int4(cur[0], cur[1], cur[2], cur[3]);
+    } else {
+        for (int64_t i = i0; i < n_sites; ++i) {
+            int32_t c = label[i], p = ld_label(label + c);
+            while (p != c) { c = p; p = ld_label(label + c); }
+            label[i] = c;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_validate(int64_t n_sites, int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
+           unsigned long long* out_bad)
+{
+    unsigned long long bad = 0;
+    const int64_t stride = (int64_t)gridDim.x * kThreads;
+    for (int64_t b = (int64_t)blockIdx.x * kThreads + threadIdx.x; b < n_bonds; b += stride) {
+        const int64_t u = src[b], v = dst[b];
+        bad += (u < 0 || u >= n_sites || v < 0 || v >= n_sites);
+    }
+    for (int o = 16; o > 0; o >>= 1) bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(out_bad, bad);
+}
+
+// ------------------------------------------------------------------------------------------------- host side
+static int check_args(int64_t n_sites, int64_t n_bonds, const void* src, const void* dst, const void* labels)
+{
+    CCL_REQUIRE(n_sites >= 0, "n_sites < 0");
+    CCL_REQUIRE(n_sites <= 2147483647LL, "n_sites > 2^31-1 (labels are int32)");
+    CCL_REQUIRE(n_bonds >= 0, "n_bonds < 0");
+    CCL_REQUIRE(n_sites == 0 || labels != nullptr, "labels is NULL");
+    CCL_REQUIRE(n_bonds == 0 || (src != nullptr && dst != nullptr), "src/dst is NULL with n_bonds > 0");
+    CCL_REQUIRE(n_bonds == 0 || n_sites > 0, "bonds given but n_sites == 0");
+    CCL_REQUIRE((reinterpret_cast<uintptr_t>(labels) & 3) == 0, "labels is not 4-byte aligned");
+    return CCL_OK;
+}
+
+template <int MASK>
+static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
+                         int32_t* labels, cudaStream_t st)
+{
+    const int64_t groups = (n_bonds + 3) / 4;
+    const int64_t blocks = (groups + kThreads - 1) / kThreads;
+    if (blocks > 2147483647LL) { set_error("n_bonds too large for one launch"); return CCL_UNSUPPORTED; }
+    uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
+    bool vec = (a & 15) == 0;
+    if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
+    if (MASK == 2 && (reinterpret_cast<uintptr_t>(occ) & 3) != 0) {
+        set_error("invalid argument: occupied_bits is not 4-byte aligned");
+        return CCL_INVALID_ARG;
+    }
+    if (vec) k_reduce<MASK, true><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels);
+    else     k_reduce<MASK, false><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels);
+    CCL_CHECK_LAUNCH("k_reduce");
+    return CCL_OK;
+}
+
+// Optional per-step CUDA events (ccl_set_profile_events): recorded on the call's stream between the kernels so
+// that a benchmark can read each step's device time from inside its own timed region.
+static thread_local cudaEvent_t g_ev[3] = {nullptr, nullptr, nullptr};
+
+static inline void mark(int k, cudaStream_t st)
+{
+    if (g_ev[k]) cudaEventRecord(g_ev[k], st);
+}
+
+static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
+                      int mask_kind, int32_t* labels, cudaStream_t st)
+{
+    int rc = check_args(n_sites, n_bonds, src, dst, labels);
+    if (rc != CCL_OK) return rc;
+    if (n_sites == 0) return CCL_OK;
+    const bool lab_vec = (reinterpret_cast<uintptr_t>(labels) & 15) == 0;
+    if (!lab_vec) { set_error("labels must be 16-byte aligned"); return CCL_UNSUPPORTED; }
+
+    const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
+    const int64_t init_blocks = site_blocks < (int64_t)kSMs * 32 ? site_blocks : (int64_t)kSMs * 32;
+    k_init<<<(unsigned)init_blocks, kThreads, 0, st>>>(n_sites, labels);                      // step (i)
+    CCL_CHECK_LAUNCH("k_init");
+    // step (ii): nothing to do after label[i] = i (every site is a root).
+    mark(0, st);
+    if (n_bonds > 0) {
+        if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, st);      // step (iii)
+        else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, st);
+        else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, st);
+        if (rc != CCL_OK) return rc;
+        mark(1, st);
+        k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels);                 // step (iv)
+        CCL_CHECK_LAUNCH("k_flatten");
+        mark(2, st);
+    }
+    return CCL_OK;
+}
+
+}  // namespace ccl
+
+extern "C" int ccl_label(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+                         const uint8_t* occupied, int32_t* labels, void* stream)
+{
+    return ccl::label_impl(n_sites, n_bonds, src, dst, occupied, 1, labels, ccl::as_stream(stream));
+}
+
+extern "C" int ccl_label_bits(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+                              const uint32_t* occupied_bits, int32_t* labels, void* stream)
+{
+    return ccl::label_impl(n_sites, n_bonds, src, dst, occupied_bits, 2, labels, ccl::as_stream(stream));
+}
+
+extern "C" int ccl_set_profile_events(void* after_init, void* after_reduce, void* after_flatten)
+{
+    ccl::g_ev[0] = static_cast<cudaEvent_t>(after_init);
+    ccl::g_ev[1] = static_cast<cudaEvent_t>(after_reduce);
+    ccl::g_ev[2] = static_cast<cudaEvent_t>(after_flatten);
+    return CCL_OK;
+}
+
+extern "C" int ccl_validate_bonds(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+                                  int64_t* out_bad, void* stream)
+{
+    using namespace ccl;
+    CCL_REQUIRE(n_sites >= 0 && n_bonds >= 0, "negative count");
+    CCL_REQUIRE(out_bad != nullptr, "out_bad is NULL");
+    CCL_REQUIRE(n_bonds == 0 || (src && dst), "src/dst is NULL with n_bonds > 0");
+    cudaStream_t st = as_stream(stream);
+    CCL_CUDA_TRY(cudaMemsetAsync(out_bad, 0, sizeof(int64_t), st));
+    if (n_bonds == 0) return CCL_OK;
+    int64_t blocks = (n_bonds + kThreads - 1) / kThreads;
+    if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+    k_validate<<<(unsigned)blocks, kThreads, 0, st>>>(n_sites, n_bonds, src, dst,
+                                                      reinterpret_cast<unsigned long long*>(out_bad));
+    CCL_CHECK_LAUNCH("k_validate");
+    return CCL_OK;
+}
+
+extern "C" int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_src,
+                                   const int32_t* host_dst, const uint32_t* host_occupied_bits,
+                                   int32_t* host_labels, void* stream)
+{
+    using namespace ccl;
+    int rc = check_args(n_sites, n_bonds, host_src, host_dst, host_labels);
+    if (rc != CCL_OK) return rc;
+    if (n_sites == 0) return CCL_OK;
+    cudaStream_t st = as_stream(stream);
+    const size_t bond_bytes = (size_t)n_bonds * sizeof(int32_t);
+    const size_t mask_bytes = host_occupied_bits ? (size_t)((n_bonds + 31) / 32) * sizeof(uint32_t) : 0;
+    const size_t label_bytes = (size_t)n_sites * sizeof(int32_t);
+    int32_t *d_src = nullptr, *d_dst = nullptr, *d_labels = nullptr;
+    uint32_t* d_bits = nullptr;
+    CCL_CUDA_TRY(cudaMallocAsync(&d_labels, label_bytes, st));
+    if (n_bonds > 0) {
+        CCL_CUDA_TRY(cudaMallocAsync(&d_src, bond_bytes, st));
+        CCL_CUDA_TRY(cudaMallocAsync(&d_dst, bond_bytes, st));
+        CCL_CUDA_TRY(cudaMemcpyAsync(d_src, host_src, bond_bytes, cudaMemcpyHostToDevice, st));
+        CCL_CUDA_TRY(cudaMemcpyAsync(d_dst, host_dst, bond_bytes, cudaMemcpyHostToDevice, st));
+        if (mask_bytes) {
+            CCL_CUDA_TRY(cudaMallocAsync(&d_bits, mask_bytes, st));
+            CCL_CUDA_TRY(cudaMemcpyAsync(d_bits, host_occupied_bits, mask_bytes, cudaMemcpyHostToDevice, st));
+        }
+    }
+    rc = label_impl(n_sites, n_bonds, d_src, d_dst, d_bits, 2, d_labels, st);
+    if (rc == CCL_OK) {
+        CCL_CUDA_TRY(cudaMemcpyAsync(host_labels, d_labels, label_bytes, cudaMemcpyDeviceToHost, st));
+    }
+    if (d_bits) cudaFreeAsync(d_bits, st);
+    if (d_dst) cudaFreeAsync(d_dst, st);
+    if (d_src) cudaFreeAsync(d_src, st);
+    cudaFreeAsync(d_labels, st);
+    CCL_CUDA_TRY(cudaStreamSynchronize(st));
+    return rc;
+}

@@ -1,0 +1,103 @@
+"""Device generators and the statistics reducer against the oracle's CPU versions: bit-exact integers."""
+import numpy as np
+import pytest
+import torch
+
+import graphs
+from oracle import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ccl():
+    import paper_1603_08357_b200 as pkg
+    assert torch.cuda.is_available()
+    return pkg
+
+
+@pytest.mark.parametrize("L", [1, 2, 3, 7, 64, 257])
+def test_lattice_generators(ccl, L):
+    for dev_gen, cpu_gen in ((ccl.gen_triangular, oracle.gen_triangular), (ccl.gen_honeycomb, oracle.gen_honeycomb)):
+        s, d = dev_gen(L)
+        ws, wd = cpu_gen(L)
+        assert np.array_equal(s.cpu().numpy(), ws) and np.array_equal(d.cpu().numpy(), wd)
+
+
+@pytest.mark.parametrize("m,p,r", [(1, 0.5, 0), (31, 0.5, 1), (32, 0.3473, 0), (33, 0.6527, 2), (1003, 1 / 3, 0),
+                                   (12288, 0.6527, 0), (1 << 20, 0.45, 7), (77, 0.0, 0), (77, 1.0, 0), (77, 1.5, 0)])
+def test_occupancy_generator(ccl, m, p, r):
+    seed = oracle.seed_for(1)
+    mask, bits = ccl.gen_occupancy(m, p, seed, r)
+    wm, wb = oracle.gen_occupancy(m, p, seed, r)
+    assert np.array_equal(mask.cpu().numpy(), wm)
+    assert np.array_equal(bits.cpu().numpy().view(np.uint32), wb)
+    only_bits = ccl.gen_occupancy(m, p, seed, r, want_mask=False)[1]
+    assert torch.equal(only_bits, bits)
+
+
+@pytest.mark.parametrize("n,z,seed", [(6, 3, 6), (10, 4, 5), (64, 3, 1), (1000, 3, 2), (4096, 4, 3), (50000, 4, 4),
+                                      ((1 << 18) + 2, 3, 11), (1 << 20, 4, 12)])
+def test_regular_generator(ccl, n, z, seed):
+    s, d = ccl.gen_regular(n, z, seed)
+    ws, wd, nrep = oracle.gen_regular(n, z, seed)
+    assert np.array_equal(s.cpu().numpy(), ws) and np.array_equal(d.cpu().numpy(), wd)
+
+
+def test_regular_generator_repairs_defects(ccl):
+    """Make sure the comparison above exercises the repair path: among these seeds several graphs need repairs."""
+    total = 0
+    for seed in range(100, 110):
+        s, d = ccl.gen_regular(2000, 4, seed)
+        ws, wd, nrep = oracle.gen_regular(2000, 4, seed)
+        total += nrep
+        assert np.array_equal(s.cpu().numpy(), ws) and np.array_equal(d.cpu().numpy(), wd)
+    assert total >= 10
+
+
+@pytest.mark.parametrize("case", ["identity", "one", "honeycomb", "regular4_giant", "tiny"])
+def test_cluster_stats(ccl, case):
+    if case == "identity":
+        labels = np.arange(1000, dtype=np.int32)
+    elif case == "one":
+        labels = np.zeros(100000, dtype=np.int32)
+    elif case == "tiny":
+        labels = np.array([0, 0, 2, 2, 4], dtype=np.int32)       # tie between clusters 0 and 2 -> label 0
+    elif case == "honeycomb":
+        L = 200
+        src, dst = oracle.gen_honeycomb(L)
+        mask, _ = oracle.gen_occupancy(src.size, 0.6527, oracle.seed_for(3))
+        labels = oracle.label(2 * L * L, src, dst, mask)
+    else:
+        n = 1 << 19
+        src, dst, _ = oracle.gen_regular(n, 4, oracle.seed_for(5))
+        mask, _ = oracle.gen_occupancy(src.size, 0.45, oracle.seed_for(5))
+        labels = oracle.label(n, src, dst, mask)
+    n_dense = 64
+    want, whd, whl = oracle.stats(labels, n_dense)
+    got, hd, hl = ccl.cluster_stats(torch.from_numpy(labels).cuda(), n_dense)
+    assert got == want
+    assert np.array_equal(hd.numpy(), whd) and np.array_equal(hl.numpy(), whl)
+    # derived floats come from exact integers on both sides -> identical (north_star: 1e-12 relative)
+    n = labels.size
+    for f in (lambda s: s["largest"] / n, lambda s: (s["sum_s2"] - s["largest"] ** 2) / n):
+        a, b = f(got), f(want)
+        assert abs(a - b) <= 1e-12 * max(abs(b), 1e-300)
+
+
+def test_cluster_stats_empty(ccl):
+    got, hd, hl = ccl.cluster_stats(torch.zeros(0, dtype=torch.int32, device="cuda"), 4)
+    assert got == dict(n_clusters=0, largest=0, largest_label=-1, sum_s2=0)
+
+
+def test_pipeline_on_device_matches_oracle_pipeline(ccl):
+    """Device generators -> ccl_label_bits -> ccl_cluster_stats, against the oracle doing the same on the CPU."""
+    L = 128
+    s, d = ccl.gen_triangular(L)
+    _, bits = ccl.gen_occupancy(3 * L * L, 0.3473, oracle.seed_for(2), 3, want_mask=False)
+    lab = ccl.label_bits(L * L, s, d, bits)
+    ws, wd = oracle.gen_triangular(L)
+    wm, _ = oracle.gen_occupancy(3 * L * L, 0.3473, oracle.seed_for(2), 3)
+    wl = oracle.label(L * L, ws, wd, wm)
+    assert np.array_equal(lab.cpu().numpy(), wl)
+    assert ccl.cluster_stats(lab)[0] == oracle.stats(wl)[0]

@@ -1,0 +1,208 @@
+"""Parity of the CUDA path (through the C ABI of libccl.so) with the CPU oracle, element by element, on the same
+seeded inputs.  Integer work: the bar is bit-exact.  Inputs always come from the oracle-side generators or from
+tests/graphs.py (never from the CUDA path); the device generators are compared against the oracle's separately."""
+import numpy as np
+import pytest
+import torch
+
+import graphs
+from oracle import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ccl():
+    import paper_1603_08357_b200 as pkg
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device; there is no CPU fallback"
+    return pkg
+
+
+def dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.view(dtype)
+    return t.cuda()
+
+
+def bits_dev(bits):
+    return dev(bits.view(np.int32))
+
+
+def run_all_forms(ccl, n, src, dst, mask):
+    """labels through ccl_label (uint8 mask) and ccl_label_bits (packed); both must equal the oracle's."""
+    want = oracle.label(n, src, dst, mask)
+    s, d = dev(src), dev(dst)
+    got8 = ccl.label(n, s, d, None if mask is None else dev(mask)).cpu().numpy()
+    assert np.array_equal(got8, want)
+    if mask is not None:
+        gotb = ccl.label_bits(n, s, d, bits_dev(graphs.pack_bits(mask))).cpu().numpy()
+        assert np.array_equal(gotb, want)
+    return want
+
+
+# ------------------------------------------------------------------ the paper's example and tiny graphs
+def test_fig1_example(ccl):
+    nn = graphs.read_fig1_nn_list()
+    want, _ = graphs.read_e0_labels()
+    src, dst = graphs.bonds_from_nn_list(nn)
+    got = ccl.label(22, dev(src), dev(dst)).cpu().tolist()
+    assert got == want["fig4_right"]                       # PAPER.md:95-107, Fig. 4 right
+
+
+def test_random_small_graphs(ccl):
+    rng = np.random.default_rng(8357)
+    for trial in range(120):
+        n = int(rng.integers(1, 200))
+        m = int(rng.integers(0, 4 * n + 1))
+        src, dst = graphs.random_graph(rng, n, m, self_loops=True)
+        mask = (rng.random(m) < rng.random()).astype(np.uint8)
+        if m == 0:
+            got = ccl.label(n, dev(src), dev(dst)).cpu().numpy()
+            assert np.array_equal(got, np.arange(n))
+            continue
+        want = run_all_forms(ccl, n, src, dst, mask)
+        assert np.array_equal(want, graphs.bfs_min_labels(n, src, dst, mask))
+
+
+def test_edge_cases(ccl):
+    e = torch.zeros(0, dtype=torch.int32, device="cuda")
+    assert ccl.label(0, e, e).numel() == 0
+    assert ccl.label(1, e, e).cpu().tolist() == [0]
+    assert ccl.label(7, e, e).cpu().tolist() == list(range(7))
+    assert ccl.label_bits(7, e, e, None).cpu().tolist() == list(range(7))
+    src = dev(np.array([2, 2, 3, 3, 0, 0, 0], dtype=np.int32))
+    dst = dev(np.array([2, 4, 3, 3, 1, 1, 1], dtype=np.int32))          # self-loops, duplicates
+    assert ccl.label(5, src, dst).cpu().tolist() == [0, 0, 2, 3, 2]
+    assert ccl.label(5, src, dst, torch.zeros(7, dtype=torch.uint8, device="cuda")).cpu().tolist() == [0, 1, 2, 3, 4]
+    assert ccl.validate_bonds(5, src, dst) == 0 and ccl.validate_bonds(4, src, dst) == 1
+    # labels need no initial content
+    lab = torch.full((5,), -12345, dtype=torch.int32, device="cuda")
+    ccl.label(5, src, dst, labels=lab)
+    assert lab.cpu().tolist() == [0, 0, 2, 3, 2]
+
+
+@pytest.mark.parametrize("m", [1, 2, 3, 4, 5, 31, 32, 33, 127, 1023, 1025, 4099])
+def test_ragged_tails_and_unaligned_pointers(ccl, m):
+    rng = np.random.default_rng(m)
+    n = max(2, m // 2)
+    src, dst = graphs.random_graph(rng, n, m)
+    mask = (rng.random(m) < 0.7).astype(np.uint8)
+    want = run_all_forms(ccl, n, src, dst, mask)
+    # unaligned views: element offset 1 breaks the 16-byte alignment of src/dst and the 4-byte alignment of the mask
+    s = dev(np.concatenate([[0], src]).astype(np.int32))[1:]
+    d = dev(np.concatenate([[0], dst]).astype(np.int32))[1:]
+    o = dev(np.concatenate([[1], mask]).astype(np.uint8))[1:]
+    assert np.array_equal(ccl.label(n, s, d, o).cpu().numpy(), want)
+    assert np.array_equal(ccl.label_bits(n, s, d, bits_dev(graphs.pack_bits(mask))).cpu().numpy(), want)
+    # garbage in the unused high bits of the last mask word must be ignored
+    bits = graphs.pack_bits(mask).copy()
+    if m % 32:
+        bits[-1] |= np.uint32(0xFFFFFFFF) << np.uint32(m % 32)
+    assert np.array_equal(ccl.label_bits(n, dev(src), dev(dst), bits_dev(bits)).cpu().numpy(), want)
+
+
+@pytest.mark.parametrize("order", ["ascending", "descending", "shuffled"])
+def test_path_graph_worst_case_depth(ccl, order):
+    rng = np.random.default_rng(5)
+    n = 1 << 20
+    src, dst = graphs.path_graph(n, order, rng)
+    got = ccl.label(n, dev(src), dev(dst))
+    assert int(got.max().item()) == 0
+    perm = rng.permutation(src.size)
+    got = ccl.label(n, dev(src[perm]), dev(dst[perm]))
+    assert int(got.max().item()) == 0
+
+
+def test_star_and_clique_contention(ccl):
+    n = 1 << 16
+    hub = np.full(n - 1, n - 1, dtype=np.int32)              # every bond hits the highest-numbered site
+    leaves = np.arange(n - 1, dtype=np.int32)
+    assert int(ccl.label(n, dev(hub), dev(leaves)).max().item()) == 0
+    k = 300
+    iu = np.triu_indices(k, 1)
+    src, dst = iu[1].astype(np.int32) + 5, iu[0].astype(np.int32) + 5
+    got = ccl.label(k + 10, dev(src), dev(dst)).cpu().numpy()
+    assert np.array_equal(got, oracle.label(k + 10, src, dst))
+
+
+# ------------------------------------------------------------------ the benchmark workloads, several tiles + tails
+def _case(name):
+    if name == "cfg1_honeycomb_L64":
+        L = 64; src, dst = oracle.gen_honeycomb(L); return 2 * L * L, src, dst, [0.6527], 1
+    if name == "honeycomb_L301":
+        L = 301; src, dst = oracle.gen_honeycomb(L); return 2 * L * L, src, dst, [0.60, 0.6527, 0.70], 3
+    if name == "triangular_L257":
+        L = 257; src, dst = oracle.gen_triangular(L); return L * L, src, dst, [0.3473 / 2, 0.3473, 0.52], 2
+    if name == "regular3":
+        n = (1 << 18) + 2; src, dst, _ = oracle.gen_regular(n, 3, oracle.seed_for(4)); return n, src, dst, [0.25, 0.5, 0.75], 4
+    if name == "regular4":
+        n = (1 << 19) + 1; src, dst, _ = oracle.gen_regular(n, 4, oracle.seed_for(5)); return n, src, dst, [0.25, 1 / 3, 0.45], 5
+    if name == "cayley_standard":
+        n, src, dst = oracle.gen_cayley3(16); return n, src, dst, [0.25, 0.5, 0.75], 6
+    if name == "cayley_random":
+        n, _, _ = oracle.gen_cayley3(16)
+        perm = np.random.default_rng(16).permutation(n).astype(np.int32)
+        n, src, dst = oracle.gen_cayley3(16, perm); return n, src, dst, [0.25, 0.5, 0.75], 7
+    raise KeyError(name)
+
+
+@pytest.mark.parametrize("name", ["cfg1_honeycomb_L64", "honeycomb_L301", "triangular_L257", "regular3", "regular4",
+                                  "cayley_standard", "cayley_random"])
+def test_workloads_bit_exact(ccl, name):
+    n, src, dst, ps, cfg = _case(name)
+    for p in ps + [0.0, 1.0]:
+        for r in range(2):
+            mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(cfg), realization=r)
+            want = run_all_forms(ccl, n, src, dst, mask)
+            if p == 0.0:
+                assert np.array_equal(want, np.arange(n))
+    # repeated calls on the same buffers give the same answer (the call leaves no state behind)
+    mask, bits = oracle.gen_occupancy(src.size, ps[-1], oracle.seed_for(cfg))
+    s, d, b = dev(src), dev(dst), bits_dev(bits)
+    lab = torch.empty(n, dtype=torch.int32, device="cuda")
+    first = ccl.label_bits(n, s, d, b, labels=lab).clone()
+    for _ in range(3):
+        assert torch.equal(ccl.label_bits(n, s, d, b, labels=lab), first)
+
+
+def test_bond_order_and_orientation_do_not_matter(ccl):
+    n, src, dst, ps, cfg = _case("regular4")
+    rng = np.random.default_rng(1)
+    mask, _ = oracle.gen_occupancy(src.size, 0.45, oracle.seed_for(cfg))
+    want = oracle.label(n, src, dst, mask)
+    perm = rng.permutation(src.size)
+    flip = rng.random(src.size) < 0.5
+    s2 = np.where(flip, dst, src)[perm].astype(np.int32)
+    d2 = np.where(flip, src, dst)[perm].astype(np.int32)
+    assert np.array_equal(ccl.label(n, dev(s2), dev(d2), dev(mask[perm])).cpu().numpy(), want)
+    order = np.argsort(np.maximum(src, dst), kind="stable")         # adversarial: all bonds of a site together
+    assert np.array_equal(ccl.label(n, dev(src[order]), dev(dst[order]), dev(mask[order])).cpu().numpy(), want)
+
+
+def test_on_a_side_stream(ccl):
+    n, src, dst, ps, cfg = _case("triangular_L257")
+    mask, bits = oracle.gen_occupancy(src.size, 0.3473, oracle.seed_for(cfg))
+    want = oracle.label(n, src, dst, mask)
+    s, d, b = dev(src), dev(dst), bits_dev(bits)
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        got = ccl.label_bits(n, s, d, b)
+    st.synchronize()
+    assert np.array_equal(got.cpu().numpy(), want)
+
+
+def test_host_buffer_entry_point(ccl):
+    n, src, dst, ps, cfg = _case("regular3")
+    mask, bits = oracle.gen_occupancy(src.size, 0.5, oracle.seed_for(cfg))
+    want = oracle.label(n, src, dst, mask)
+    hs = torch.from_numpy(src).pin_memory()
+    hd = torch.from_numpy(dst).pin_memory()
+    hb = torch.from_numpy(bits.view(np.int32)).pin_memory()
+    out = torch.empty(n, dtype=torch.int32).pin_memory()
+    ccl.label_bits_host(n, hs, hd, hb, out)
+    assert np.array_equal(out.numpy(), want)
+    out2 = torch.empty(n, dtype=torch.int32)                         # pageable memory works too
+    ccl.label_bits_host(n, torch.from_numpy(src), torch.from_numpy(dst), torch.from_numpy(bits.view(np.int32)), out2)
+    assert np.array_equal(out2.numpy(), want)
