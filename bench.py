@@ -193,6 +193,8 @@ def run_ours(args):
     fam, size, z, ps, kind, cfg = WORKLOADS[args.workload]
     n, m, text = describe(args.workload)
     seed = SEED_BASE + cfg
+    if args.region_shift >= 0 or args.force_mode >= 0:
+        ccl.set_tuning(-1, args.region_shift, args.force_mode)
     # ---- synthetic inputs, generated on the device by the library's own seeded generators (untimed)
     if fam == "regular":
         src, dst = ccl.gen_regular(n, z, seed)
@@ -356,6 +358,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--region-shift", type=int, default=-1, help="experiment: log2 sites per region of the bucketed form")
+    ap.add_argument("--force-mode", type=int, default=-1, help="experiment: -1 probe, 0 direct, 1 bucketed")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -11,7 +11,9 @@
  *
  * Conventions for every entry point
  *   - All array pointers are DEVICE pointers owned by the caller unless the name says `host_`.  The library
- *     never frees caller memory and keeps no allocation alive after a call returns.
+ *     never frees caller memory.  Scratch a call needs comes from the library's own stream-ordered memory pool
+ *     (cudaMallocFromPoolAsync) and is returned to that pool, in stream order, before the call returns; the pool
+ *     keeps the memory for the next call.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the default stream).  All work is enqueued on it; no
  *     entry point synchronises with the host unless stated.  Results are valid once the stream has drained.
  *   - Return value: CCL_OK (0) or a ccl_status.  No exception crosses the ABI.  ccl_last_error() returns a
@@ -110,6 +112,19 @@ int ccl_cluster_stats(int64_t n_sites, const int32_t* labels, int32_t* size_scra
  * frees, runs ccl_label_bits, copies labels back to host_labels and synchronises the stream before returning. */
 int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_src, const int32_t* host_dst,
                         const uint32_t* host_occupied_bits, int32_t* host_labels, void* stream);
+
+/* ---- tuning --------------------------------------------------------------------------------------------
+ *
+ * Step (iii) has two forms: the direct one-pass kernel, and a region-bucketed form for label
+ * arrays too large for L2, which a device-side probe selects when the bonds are not local in the site numbering.
+ * bucket_min_label_bytes: label arrays of at least this many bytes are eligible for the bucketed form (default
+ * 96 MiB; 0 makes every call eligible).  region_shift: a region is 2^region_shift sites (default 23; raised
+ * automatically so that there are at most 32 regions).  force_mode: -1 = probe decides, 0 = always direct,
+ * 1 = always bucketed when eligible.  bucket_capacity: pairs each region's bucket can hold (<= 0: 4 M / regions +
+ * 4096); pairs that do not fit are joined on the spot by the general algorithm.  A negative size/shift restores the default.  Process-wide; the result of
+ * ccl_label does not depend on any of this. */
+int ccl_set_tuning(int64_t bucket_min_label_bytes, int32_t region_shift, int32_t force_mode,
+                   int64_t bucket_capacity);
 
 /* ---- profiling hook ------------------------------------------------------------------------------------
  *

@@ -19,8 +19,57 @@ void set_error(const char* fmt, ...)
 
 void count_launch(int n) { g_launches += n; }
 
+Tuning& tuning()
+{
+    static Tuning t;
+    return t;
+}
+
+int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st)
+{
+    static cudaMemPool_t pools[64] = {};
+    int dev = 0;
+    CCL_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) { set_error("device index %d out of range", dev); return CCL_UNSUPPORTED; }
+    if (pools[dev] == nullptr) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        CCL_CUDA_TRY(cudaMemPoolCreate(&pool, &props));
+        unsigned long long keep = ~0ull;
+        CCL_CUDA_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        pools[dev] = pool;
+    }
+    CCL_CUDA_TRY(cudaMallocFromPoolAsync(ptr, bytes, pools[dev], st));
+    return CCL_OK;
+}
+
 }  // namespace ccl
 
 extern "C" const char* ccl_last_error(void) { return ccl::g_error; }
 extern "C" int ccl_version(void) { return 100; }      // 0.1.0
 extern "C" int64_t ccl_launch_count(void) { return ccl::g_launches; }
+
+extern "C" int ccl_set_tuning(int64_t bucket_min_label_bytes, int32_t region_shift, int32_t force_mode,
+                              int64_t bucket_capacity)
+{
+    ccl::Tuning def;
+    ccl::Tuning& t = ccl::tuning();
+    if (region_shift >= 0 && (region_shift < 4 || region_shift > 30)) {
+        ccl::set_error("invalid argument: region_shift must lie in [4, 30]");
+        return CCL_INVALID_ARG;
+    }
+    if (force_mode < -1 || force_mode > 1) {
+        ccl::set_error("invalid argument: force_mode must be -1, 0 or 1");
+        return CCL_INVALID_ARG;
+    }
+    t.bucket_min_label_bytes = bucket_min_label_bytes >= 0 ? bucket_min_label_bytes : def.bucket_min_label_bytes;
+    t.bucket_min_bonds = bucket_min_label_bytes >= 0 ? 0 : def.bucket_min_bonds;
+    t.region_shift = region_shift >= 0 ? region_shift : def.region_shift;
+    t.force_mode = force_mode;
+    t.bucket_capacity = bucket_capacity > 0 ? bucket_capacity : 0;
+    return CCL_OK;
+}

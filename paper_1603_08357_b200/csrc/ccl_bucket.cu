@@ -1,0 +1,255 @@
+// ccl_bucket.cu -- step (iii) of PAPER.md:113 for label arrays that do not fit in L2: region-bucketed label reduction.
+//
+// Why: on B200 a random atomicMin into a 256 MiB label[] runs at ~31 G/s (every access is an HBM sector fetch plus a
+// write-back), into an L2-resident 32-64 MiB slice at ~130 G/s (profiles/r1_ubench.txt).  So the site range is cut
+// into regions whose labels fit in L2, every occupied bond is filed under the region of its HIGHER endpoint, and the
+// regions are reduced one after the other from the highest down.  Within region r each pair (a, b), a < b, runs
+// Algorithm 1's atomic loop directly on its own endpoints:
+//
+//       old = atomicMin(&label[b], a)      -- b lies in region r: L2 hit
+//       old == b : b was a root, now hangs under a          -> done   (label_3 = label_1 in the paper's notation)
+//       old == a : already linked                           -> done   (label_3 = label_2)
+//       else     : the pair still to be joined is {a, old}  -> its higher site is < b
+//
+// The higher site of a pending pair only ever decreases, so a pair either stays in region r (the loop goes on in
+// the same thread) or is re-filed under a LOWER region, which has not been reduced yet.  No root finding and no
+// access outside the region are needed; after region 0 label[] is a forest with label[x] <= x, and step (iv)
+// flattens it.  Measured chain lengths: 1.3-2.2 atomics per occupied bond on random regular graphs.
+//
+// A device-side probe decides whether to take this form at all: graphs whose bonds are local in the site numbering
+// (raster-ordered lattices) keep the direct one-pass kernel of ccl_label.cu, whose gathers hit L2 anyway.
+#include "ccl_common.cuh"
+#include "ccl_unionfind.cuh"
+
+namespace ccl {
+
+constexpr int kBThreads = 256;
+
+__device__ __forceinline__ void st_stream_pair(int2* p, int2 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.s32 [%0], {%1, %2}, %3;" ::"l"(p), "r"(v.x), "r"(v.y), "l"(pol)
+                 : "memory");
+}
+
+// Shared-memory scratch of the CTA-wide append: pairs are counted per target region, one global atomicAdd per
+// region reserves the CTA's range in that bucket, and the pairs leave through a staging array so that consecutive
+// threads write consecutive addresses.
+template <int P>
+struct EmitSmem {
+    int cnt[kMaxRegions];
+    int pref[kMaxRegions + 1];
+    unsigned long long base[kMaxRegions];
+    int2 stage[kBThreads * P];
+};
+
+// Every thread hands in up to P pairs (lo[k] < 0 = none).  Must be called by all threads of the CTA.
+template <int P>
+__device__ __forceinline__ void cta_emit(EmitSmem<P>& sm, const int32_t (&lo)[P], const int32_t (&hi)[P], int shift,
+                                         BucketHeader* hdr, int2* buckets, unsigned long long cap, int32_t* label,
+                                         uint64_t pol)
+{
+    const int tid = threadIdx.x;
+    if (tid < kMaxRegions) sm.cnt[tid] = 0;
+    __syncthreads();
+    int rank[P];
+#pragma unroll
+    for (int k = 0; k < P; ++k) rank[k] = (lo[k] >= 0) ? atomicAdd(&sm.cnt[hi[k] >> shift], 1) : 0;
+    __syncthreads();
+    if (tid < 32) {
+        const int c = sm.cnt[tid];
+        int incl = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (tid >= o) incl += t;
+        }
+        sm.pref[tid] = incl - c;
+        if (tid == 31) sm.pref[32] = incl;
+        sm.base[tid] = c ? atomicAdd(&hdr->count[tid], (unsigned long long)c) : 0ull;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < P; ++k)
+        if (lo[k] >= 0) sm.stage[sm.pref[hi[k] >> shift] + rank[k]] = make_int2(lo[k], hi[k]);
+    __syncthreads();
+    const int total = sm.pref[32];
+    for (int j = tid; j < total; j += kBThreads) {
+        const int2 pr = sm.stage[j];
+        const int r = pr.y >> shift;
+        const unsigned long long pos = sm.base[r] + (unsigned long long)(j - sm.pref[r]);
+        if (pos < cap) st_stream_pair(buckets + (size_t)r * cap + pos, pr, pol);
+        else algorithm1(label, pr.x, pr.y);          // bucket full: join the pair right here, the slow general way
+    }
+    __syncthreads();
+}
+
+// ---------------------------------------------------------------------------------------------------- probe
+// Samples bonds at a fixed stride and looks at how many join two different regions.  Random numbering: 1 - 1/R of
+// them; raster-ordered lattice: only those on region borders.
+__global__ void __launch_bounds__(1024)
+k_probe(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, int shift, int force_mode,
+        BucketHeader* hdr)
+{
+    __shared__ int s_cross;
+    if (threadIdx.x == 0) s_cross = 0;
+    __syncthreads();
+    const int64_t samples = n_bonds < 8192 ? n_bonds : 8192;
+    const int64_t stride = n_bonds / samples;
+    int cross = 0;
+    for (int64_t i = threadIdx.x; i < samples; i += 1024) {
+        const int32_t u = src[i * stride], v = dst[i * stride];
+        cross += (u >> shift) != (v >> shift);
+    }
+    for (int o = 16; o > 0; o >>= 1) cross += __shfl_xor_sync(0xffffffffu, cross, o);
+    if ((threadIdx.x & 31) == 0 && cross) atomicAdd(&s_cross, cross);
+    __syncthreads();
+    if (threadIdx.x == 0) hdr->mode = force_mode >= 0 ? force_mode : ((4 * (int64_t)s_cross >= samples) ? 1 : 0);
+}
+
+// -------------------------------------------------------------------------------------------------- scatter
+// One pass over the bond stream: occupied, non-loop bonds become (lo, hi) pairs filed under region(hi).
+template <int MASK>
+__global__ void __launch_bounds__(kBThreads)
+k_scatter(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
+          const void* __restrict__ occ, int vec, int shift, BucketHeader* hdr, int2* buckets,
+          unsigned long long cap, int32_t* label)
+{
+    constexpr int P = 8;
+    __shared__ EmitSmem<P> sm;
+    if (hdr->mode != 1) return;
+    const uint64_t pol = evict_first_policy();
+    const int64_t tiles = (n_bonds + kBThreads * P - 1) / (kBThreads * P);
+    for (int64_t tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
+        const int64_t b0 = (tile * kBThreads + threadIdx.x) * P;
+        int32_t lo[P], hi[P];
+        int cnt = 0;
+        if (b0 < n_bonds) cnt = (n_bonds - b0 >= P) ? P : (int)(n_bonds - b0);
+        uint32_t m = (1u << cnt) - 1u;
+        if (cnt > 0) {
+            if (MASK == 2) {
+                m &= ld_stream_u32(static_cast<const uint32_t*>(occ) + (b0 >> 5), pol) >> (b0 & 31);   // b0 % 8 == 0
+            } else if (MASK == 1) {
+                const uint8_t* o = static_cast<const uint8_t*>(occ) + b0;
+                uint32_t mm = 0;
+                for (int k = 0; k < cnt; ++k) mm |= (uint32_t)(ld_stream_u8(o + k, pol) != 0) << k;
+                m &= mm;
+            }
+        }
+        int32_t u[P], v[P];
+        if (vec && cnt == P) {
+            const int4 s0 = ld_stream_v4(src + b0, pol), s1 = ld_stream_v4(src + b0 + 4, pol);
+            const int4 d0 = ld_stream_v4(dst + b0, pol), d1 = ld_stream_v4(dst + b0 + 4, pol);
+            u[0] = s0.x; u[1] = s0.y; u[2] = s0.z; u[3] = s0.w; u[4] = s1.x; u[5] = s1.y; u[6] = s1.z; u[7] = s1.w;
+            v[0] = d0.x; v[1] = d0.y; v[2] = d0.z; v[3] = d0.w; v[4] = d1.x; v[5] = d1.y; v[6] = d1.z; v[7] = d1.w;
+        } else {
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                u[k] = (k < cnt) ? ld_stream_s32(src + b0 + k, pol) : 0;
+                v[k] = (k < cnt) ? ld_stream_s32(dst + b0 + k, pol) : 0;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            const bool on = ((m >> k) & 1u) && u[k] != v[k];
+            lo[k] = on ? min(u[k], v[k]) : -1;
+            hi[k] = max(u[k], v[k]);
+        }
+        cta_emit<P>(sm, lo, hi, shift, hdr, buckets, cap, label, pol);
+    }
+}
+
+// -------------------------------------------------------------------------------------------------- descend
+// Reduce region r: all label[] traffic of this launch falls into [r << shift, (r+1) << shift).
+__global__ void __launch_bounds__(kBThreads)
+k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long cap, int32_t* label)
+{
+    constexpr int P = 4;
+    __shared__ EmitSmem<P> sm;
+    if (hdr->mode != 1) return;
+    const uint64_t pol = evict_first_policy();
+    unsigned long long n = hdr->count[r];
+    if (n > cap) n = cap;
+    const int2* bucket = buckets + (size_t)r * cap;
+    const long long tiles = (long long)((n + kBThreads * P - 1) / (kBThreads * P));
+    for (long long tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
+        const unsigned long long i0 = ((unsigned long long)tile * kBThreads + threadIdx.x) * P;
+        int32_t a[P], b[P], old[P];
+        if (i0 + P <= n) {
+            const int4 q0 = ld_stream_v4(reinterpret_cast<const int32_t*>(bucket + i0), pol);
+            const int4 q1 = ld_stream_v4(reinterpret_cast<const int32_t*>(bucket + i0 + 2), pol);
+            a[0] = q0.x; b[0] = q0.y; a[1] = q0.z; b[1] = q0.w; a[2] = q1.x; b[2] = q1.y; a[3] = q1.z; b[3] = q1.w;
+        } else {
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                a[k] = -1; b[k] = 0;
+                if (i0 + k < n) {
+                    a[k] = ld_stream_s32(reinterpret_cast<const int32_t*>(bucket + i0 + k), pol);
+                    b[k] = ld_stream_s32(reinterpret_cast<const int32_t*>(bucket + i0 + k) + 1, pol);
+                }
+            }
+        }
+        // first atomics of the four pairs in flight together
+#pragma unroll
+        for (int k = 0; k < P; ++k) old[k] = (a[k] >= 0) ? atomicMin(label + b[k], a[k]) : a[k];
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            int32_t aa = a[k], bb = b[k], oo = old[k];
+            bool pending = false;
+            while (aa >= 0 && oo != bb && oo != aa) {
+                const int32_t na = min(aa, oo), nb = max(aa, oo);
+                aa = na; bb = nb;
+                if ((bb >> shift) != r) { pending = true; break; }     // leaves the region: re-file it lower down
+                // Continuation steps mostly land on sites that are linked already, and the lowest sites of a big
+                // cluster are hit by millions of them: look before writing.  A (possibly stale, L1-cached) value
+                // v <= aa means the atomic would not write, and {v, aa} is the pair that is left (or nothing, if
+                // v == aa): whoever replaced v later took over the duty of joining v to its successor.
+                oo = label[bb];
+                if (oo > aa) oo = atomicMin(label + bb, aa);
+            }
+            a[k] = pending ? aa : -1;
+            b[k] = bb;
+        }
+        cta_emit<P>(sm, a, b, shift, hdr, buckets, cap, label, pol);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------- host side
+int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
+                    int mask_kind, int32_t* labels, cudaStream_t st, BucketHeader** hdr_out, void** ws_out)
+{
+    // region size: 2^23 sites (32 MiB of labels) unless that would need more than kMaxRegions regions
+    int shift = tuning().region_shift;
+    while (((n_sites - 1) >> shift) + 1 > kMaxRegions) ++shift;
+    const int n_regions = (int)(((n_sites - 1) >> shift) + 1);
+    unsigned long long cap = (unsigned long long)((4 * n_bonds) / n_regions + 4096);
+    if (tuning().bucket_capacity > 0) cap = (unsigned long long)tuning().bucket_capacity;
+    cap = (cap + 3ull) & ~3ull;                                   // keeps every bucket 32-byte aligned
+    const size_t hdr_bytes = (sizeof(BucketHeader) + 255) & ~(size_t)255;
+    const size_t bytes = hdr_bytes + (size_t)n_regions * cap * sizeof(int2);
+    void* ws = nullptr;
+    { const int rc = scratch_alloc(&ws, bytes, st); if (rc != CCL_OK) return rc; }
+    *ws_out = ws;
+    BucketHeader* hdr = static_cast<BucketHeader*>(ws);
+    int2* buckets = reinterpret_cast<int2*>(static_cast<char*>(ws) + hdr_bytes);
+    *hdr_out = hdr;
+    CCL_CUDA_TRY(cudaMemsetAsync(hdr, 0, sizeof(BucketHeader), st));
+    k_probe<<<1, 1024, 0, st>>>(n_bonds, src, dst, shift, tuning().force_mode, hdr);
+    CCL_CHECK_LAUNCH("k_probe");
+    const uintptr_t al = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
+    const int vec = (al & 15) == 0;
+    const int grid = kSMs * 6;
+    if (occ == nullptr)
+        k_scatter<0><<<grid, kBThreads, 0, st>>>(n_bonds, src, dst, nullptr, vec, shift, hdr, buckets, cap, labels);
+    else if (mask_kind == 1)
+        k_scatter<1><<<grid, kBThreads, 0, st>>>(n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels);
+    else
+        k_scatter<2><<<grid, kBThreads, 0, st>>>(n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels);
+    CCL_CHECK_LAUNCH("k_scatter");
+    for (int r = n_regions - 1; r >= 0; --r) {
+        k_descend<<<grid, kBThreads, 0, st>>>(r, shift, hdr, buckets, cap, labels);
+        CCL_CHECK_LAUNCH("k_descend");
+    }
+    return CCL_OK;
+}
+
+}  // namespace ccl

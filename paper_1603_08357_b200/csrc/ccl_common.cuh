@@ -47,6 +47,34 @@ inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s
         }                                                                                          \
     } while (0)
 
+// ---- region-bucketed label reduction (ccl_bucket.cu) -----------------------------------------------------
+constexpr int kMaxRegions = 32;
+
+struct BucketHeader {                              // lives in device memory at the head of the call's workspace
+    int32_t mode;                                  // written by k_probe: 0 = direct one-pass kernel, 1 = bucketed
+    int32_t pad;
+    unsigned long long count[kMaxRegions];         // pairs filed under each region (may exceed the capacity: the
+                                                   // excess was joined on the spot by the general algorithm)
+};
+
+struct Tuning {                                    // ccl_set_tuning(); process-wide
+    int64_t bucket_min_label_bytes = 96ll << 20;   // label[] beyond this cannot stay resident in the 126 MB L2
+    int64_t bucket_min_bonds = 1 << 20;
+    int32_t region_shift = 23;                     // 2^23 sites = 32 MiB of labels per region
+    int32_t force_mode = -1;                       // -1: device-side probe decides; 0: direct; 1: bucketed
+    int64_t bucket_capacity = 0;                   // pairs per region bucket; 0 = 4 M / regions + 4096
+};
+Tuning& tuning();
+
+// The library's own stream-ordered memory pool on the current device (created on first use, release threshold
+// unlimited, so scratch freed by one call is reused by the next instead of going back to the driver).
+int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st);
+
+// Enqueues probe + scatter + one descend launch per region.  *ws_out is a cudaMallocAsync allocation the caller
+// frees (cudaFreeAsync) after the kernels that read *hdr_out have been enqueued.
+int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
+                    int mask_kind, int32_t* labels, cudaStream_t st, BucketHeader** hdr_out, void** ws_out);
+
 // ---- device helpers --------------------------------------------------------------------------------------
 // Streaming (read-once) loads: bypass L1 allocation and mark the L2 line evict-first, so that the bond stream
 // does not push label[] sectors out of L2.

@@ -9,6 +9,7 @@
 // Everything is integer work on int32 labels; the bound is HBM / L2 gather traffic, so there are no tensor cores
 // here.
 #include "ccl_common.cuh"
+#include "ccl_unionfind.cuh"
 
 namespace ccl {
 
@@ -28,54 +29,15 @@ __global__ void __launch_bounds__(kThreads) k_init(int64_t n_sites, int32_t* __r
     }
 }
 
-// ------------------------------------------------------------------------------------------ root finding
-// Walk label[label[...]] to the root, halving the path on the way: every visited site is
-// re-pointed at its grandparent.  A shortcut store can only write an ancestor, so it never disconnects anything
-// (DESIGN.md "Concurrency").
-__device__ __forceinline__ int32_t find_root(int32_t* label, int32_t x)
-{
-    int32_t p = ld_label(label + x);
-    while (p != x) {
-        const int32_t gp = ld_label(label + p);
-        if (gp == p) return p;
-        st_label(label + x, gp);
-        x = gp;
-        p = ld_label(label + x);
-    }
-    return x;
-}
-
-// Algorithm 1 (reading R3 of its garbled last lines, exit test R4): make sure sites a and b end
-// up in one tree.  label_1 is the larger of the two current representatives, label_2 the smaller.
-__device__ __forceinline__ void algorithm1(int32_t* label, int32_t a, int32_t b)
-{
-    int32_t label_1 = find_root(label, a);
-    int32_t label_2 = find_root(label, b);
-    while (label_1 != label_2) {
-        if (label_1 < label_2) { const int32_t t = label_1; label_1 = label_2; label_2 = t; }
-        const int32_t label_3 = atomicMin(label + label_1, label_2);
-        if (label_3 == label_1 || label_3 == label_2) return;     // linked now / was linked already
-        // label_1 was not a root any more.  If label_3 > label_2 the link label_1 -> label_3 has just been
-        // replaced by label_1 -> label_2, so label_3 must be joined to label_2; if label_3 < label_2 nothing was
-        // written and label_1 hangs under label_3, which must be joined to label_2.  Either way the pair to join
-        // is (label_3, label_2); walk both up to their roots before the next atomic.
-        label_1 = find_root(label, label_3);
-        label_2 = find_root(label, label_2);
-    }
-}
-
 // ---------------------------------------------------------------------------------------------- step (iii)
 // MASK: 0 = every bond occupied, 1 = uint8 per bond, 2 = packed bits.  VEC: src/dst 16-byte aligned (and the
 // uint8 mask 4-byte aligned), so a thread fetches its 4 bonds with two 128-bit loads.
 template <int MASK, bool VEC>
-__global__ void __launch_bounds__(kThreads)
-k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-         const void* __restrict__ occ, int32_t* label)
+__device__ __forceinline__ void reduce4(int64_t n_bonds, int64_t b0, const int32_t* __restrict__ src,
+                                        const int32_t* __restrict__ dst, const void* __restrict__ occ,
+                                        int32_t* label, uint64_t pol)
 {
-    const int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
-    if (b0 >= n_bonds) return;
     const int cnt = (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
-    const uint64_t pol = evict_first_policy();
 
     // occupancy of this thread's 4 bonds -> low 4 bits of m
     uint32_t m = 0xFu;
@@ -125,6 +87,18 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
 #pragma unroll
     for (int k = 0; k < 4; ++k)
         if (old[k] != lo[k]) algorithm1(label, old[k], lo[k]);
+}
+
+template <int MASK, bool VEC>
+__global__ void __launch_bounds__(kThreads)
+k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
+         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr)
+{
+    if (hdr != nullptr && hdr->mode == 1) return;          // the bucketed form (ccl_bucket.cu) did step (iii)
+    const uint64_t pol = evict_first_policy();
+    const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
+    for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_bonds; b0 += stride)
+        reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol);
 }
 
 // ----------------------------------------------------------------------------------------------- step (iv)
@@ -188,11 +162,11 @@ static int check_args(int64_t n_sites, int64_t n_bonds, const void* src, const v
 
 template <int MASK>
 static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                         int32_t* labels, cudaStream_t st)
+                         int32_t* labels, const BucketHeader* hdr, cudaStream_t st)
 {
     const int64_t groups = (n_bonds + 3) / 4;
-    const int64_t blocks = (groups + kThreads - 1) / kThreads;
-    if (blocks > 2147483647LL) { set_error("n_bonds too large for one launch"); return CCL_UNSUPPORTED; }
+    int64_t blocks = (groups + kThreads - 1) / kThreads;
+    if (blocks > (int64_t)kSMs * 8 * 16) blocks = (int64_t)kSMs * 8 * 16;     // grid-stride beyond 16 waves of 8 CTAs/SM
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     bool vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
@@ -200,8 +174,8 @@ static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst
         set_error("invalid argument: occupied_bits is not 4-byte aligned");
         return CCL_INVALID_ARG;
     }
-    if (vec) k_reduce<MASK, true><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels);
-    else     k_reduce<MASK, false><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels);
+    if (vec) k_reduce<MASK, true><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels, hdr);
+    else     k_reduce<MASK, false><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels, hdr);
     CCL_CHECK_LAUNCH("k_reduce");
     return CCL_OK;
 }
@@ -231,9 +205,19 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
     // step (ii): nothing to do after label[i] = i (every site is a root).
     mark(0, st);
     if (n_bonds > 0) {
-        if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, st);      // step (iii)
-        else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, st);
-        else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, st);
+        // step (iii).  Label arrays that cannot stay in L2 get the region-bucketed form if a device-side probe finds
+        // the bonds non-local in the site numbering; the direct kernel then returns at once (and vice versa).
+        BucketHeader* hdr = nullptr;
+        void* ws = nullptr;
+        if (tuning().force_mode != 0 && n_sites * (int64_t)sizeof(int32_t) >= tuning().bucket_min_label_bytes &&
+            n_bonds >= tuning().bucket_min_bonds) {
+            rc = bucketed_reduce(n_sites, n_bonds, src, dst, occ, mask_kind, labels, st, &hdr, &ws);
+            if (rc != CCL_OK) { if (ws) cudaFreeAsync(ws, st); return rc; }
+        }
+        if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, hdr, st);
+        else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, hdr, st);
+        else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, hdr, st);
+        if (ws) cudaFreeAsync(ws, st);
         if (rc != CCL_OK) return rc;
         mark(1, st);
         k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels);                 // step (iv)
@@ -297,14 +281,14 @@ extern "C" int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32
     const size_t label_bytes = (size_t)n_sites * sizeof(int32_t);
     int32_t *d_src = nullptr, *d_dst = nullptr, *d_labels = nullptr;
     uint32_t* d_bits = nullptr;
-    CCL_CUDA_TRY(cudaMallocAsync(&d_labels, label_bytes, st));
+    if ((rc = scratch_alloc((void**)&d_labels, label_bytes, st)) != CCL_OK) return rc;
     if (n_bonds > 0) {
-        CCL_CUDA_TRY(cudaMallocAsync(&d_src, bond_bytes, st));
-        CCL_CUDA_TRY(cudaMallocAsync(&d_dst, bond_bytes, st));
+        if ((rc = scratch_alloc((void**)&d_src, bond_bytes, st)) != CCL_OK) return rc;
+        if ((rc = scratch_alloc((void**)&d_dst, bond_bytes, st)) != CCL_OK) return rc;
         CCL_CUDA_TRY(cudaMemcpyAsync(d_src, host_src, bond_bytes, cudaMemcpyHostToDevice, st));
         CCL_CUDA_TRY(cudaMemcpyAsync(d_dst, host_dst, bond_bytes, cudaMemcpyHostToDevice, st));
         if (mask_bytes) {
-            CCL_CUDA_TRY(cudaMallocAsync(&d_bits, mask_bytes, st));
+            if ((rc = scratch_alloc((void**)&d_bits, mask_bytes, st)) != CCL_OK) return rc;
             CCL_CUDA_TRY(cudaMemcpyAsync(d_bits, host_occupied_bits, mask_bytes, cudaMemcpyHostToDevice, st));
         }
     }

@@ -206,3 +206,65 @@ def test_host_buffer_entry_point(ccl):
     out2 = torch.empty(n, dtype=torch.int32)                         # pageable memory works too
     ccl.label_bits_host(n, torch.from_numpy(src), torch.from_numpy(dst), torch.from_numpy(bits.view(np.int32)), out2)
     assert np.array_equal(out2.numpy(), want)
+
+
+# ------------------------------------------------------------------ region-bucketed form of step (iii)
+@pytest.fixture
+def bucketed(ccl):
+    """Force the bucketed form on small inputs: every call eligible, 2^10..2^14-site regions."""
+    yield ccl
+    ccl.set_tuning()                                   # restore defaults
+
+
+@pytest.mark.parametrize("shift,cap", [(10, 0), (12, 0), (14, 0), (12, 64), (16, 1000)])
+def test_bucketed_form_random_small_graphs(bucketed, shift, cap):
+    ccl = bucketed
+    ccl.set_tuning(0, shift, 1, cap)                   # cap > 0: tiny buckets, most pairs take the overflow path
+    rng = np.random.default_rng(shift * 131 + cap)
+    for trial in range(40):
+        n = int(rng.integers(2, 60000))
+        m = int(rng.integers(1, 3 * n + 1))
+        src, dst = graphs.random_graph(rng, n, m, self_loops=True)
+        mask = (rng.random(m) < rng.random()).astype(np.uint8)
+        run_all_forms(ccl, n, src, dst, mask)
+        assert np.array_equal(ccl.label(n, dev(src), dev(dst)).cpu().numpy(), oracle.label(n, src, dst))
+
+
+@pytest.mark.parametrize("name", ["cfg1_honeycomb_L64", "honeycomb_L301", "triangular_L257", "regular3", "regular4",
+                                  "cayley_standard", "cayley_random"])
+@pytest.mark.parametrize("mode", [1, -1])
+def test_bucketed_form_workloads_bit_exact(bucketed, name, mode):
+    ccl = bucketed
+    n, src, dst, ps, cfg = _case(name)
+    ccl.set_tuning(0, 15, mode, 0)                     # 2^15-site regions; mode -1 lets the device probe choose
+    for p in ps + [1.0]:
+        mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(cfg), realization=5)
+        run_all_forms(ccl, n, src, dst, mask)
+
+
+def test_bucketed_form_adversarial(bucketed):
+    ccl = bucketed
+    ccl.set_tuning(0, 12, 1, 0)
+    rng = np.random.default_rng(99)
+    n = 1 << 17
+    for order in ("ascending", "descending", "shuffled"):
+        src, dst = graphs.path_graph(n, order, rng)
+        assert int(ccl.label(n, dev(src), dev(dst)).max().item()) == 0
+    hub = np.full(n - 1, n - 1, dtype=np.int32)        # star on the highest site: every pair lands in one bucket
+    leaves = np.arange(n - 1, dtype=np.int32)
+    assert int(ccl.label(n, dev(hub), dev(leaves)).max().item()) == 0
+    # interleaved path 0, n/2, 1, n/2+1, ...: every bond crosses regions and the lower half becomes one long chain
+    half = n // 2
+    i = np.arange(half - 1, dtype=np.int32)
+    src = np.concatenate([i, i + half]).astype(np.int32)
+    dst = np.concatenate([i + half, i + 1]).astype(np.int32)
+    got = ccl.label(n, dev(src), dev(dst)).cpu().numpy()
+    assert np.array_equal(got, oracle.label(n, src, dst))
+
+
+def test_tuning_argument_checks(ccl):
+    with pytest.raises(ccl.CclError):
+        ccl.set_tuning(0, 2, 0)
+    with pytest.raises(ccl.CclError):
+        ccl.set_tuning(0, 12, 5)
+    ccl.set_tuning()
