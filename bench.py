@@ -195,6 +195,9 @@ def run_ours(args):
     seed = SEED_BASE + cfg
     if args.region_shift >= 0 or args.force_mode >= 0:
         ccl.set_tuning(-1, args.region_shift, args.force_mode)
+    for kv in args.option:
+        k, v = kv.split("=")
+        ccl.set_option(k, int(v))
     # ---- synthetic inputs, generated on the device by the library's own seeded generators (untimed)
     if fam == "regular":
         src, dst = ccl.gen_regular(n, z, seed)
@@ -360,6 +363,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--region-shift", type=int, default=-1, help="experiment: log2 sites per region of the bucketed form")
     ap.add_argument("--force-mode", type=int, default=-1, help="experiment: -1 probe, 0 direct, 1 bucketed")
+    ap.add_argument("--option", action="append", default=[], help="experiment: name=value for ccl_set_option")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

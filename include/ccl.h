@@ -115,16 +115,19 @@ int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_sr
 
 /* ---- tuning --------------------------------------------------------------------------------------------
  *
- * Step (iii) has two forms: the direct one-pass kernel, and a region-bucketed form for label
- * arrays too large for L2, which a device-side probe selects when the bonds are not local in the site numbering.
- * bucket_min_label_bytes: label arrays of at least this many bytes are eligible for the bucketed form (default
- * 96 MiB; 0 makes every call eligible).  region_shift: a region is 2^region_shift sites (default 23; raised
- * automatically so that there are at most 32 regions).  force_mode: -1 = probe decides, 0 = always direct,
- * 1 = always bucketed when eligible.  bucket_capacity: pairs each region's bucket can hold (<= 0: 4 M / regions +
- * 4096); pairs that do not fit are joined on the spot by the general algorithm.  A negative size/shift restores the default.  Process-wide; the result of
- * ccl_label does not depend on any of this. */
-int ccl_set_tuning(int64_t bucket_min_label_bytes, int32_t region_shift, int32_t force_mode,
-                   int64_t bucket_capacity);
+ * ccl_set_option(name, value): process-wide knobs; none of them changes the result of ccl_label.  Step (iii) has two
+ * forms: the direct one-pass kernel, and a region-bucketed form for label arrays too large for
+ * L2, which a device-side probe selects when the bonds are not local in the site numbering.
+ *   "bucket_min_label_bytes"  label arrays of at least this many bytes are eligible for the bucketed form
+ *                             (default 96 MiB; 0 makes every call eligible; negative restores the default)
+ *   "region_shift"            a region is 2^value sites (default 23, allowed 4..30; raised automatically so that
+ *                             there are at most 32 regions; negative restores the default)
+ *   "force_mode"              -1 = the probe decides (default), 0 = always direct, 1 = always bucketed when eligible
+ *   "bucket_capacity"         pairs each region's bucket can hold (<= 0: 4 M / regions + 4096); pairs that do not
+ *                             fit are joined on the spot by the general algorithm
+ *   "reset"                   all defaults (value ignored)
+ * Unknown names -> CCL_INVALID_ARG. */
+int ccl_set_option(const char* name, int64_t value);
 
 /* ---- profiling hook ------------------------------------------------------------------------------------
  *

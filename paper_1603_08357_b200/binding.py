@@ -14,7 +14,7 @@ lib = C.CDLL(_LIB_PATH)
 
 EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangular", "ccl_gen_honeycomb",
            "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
-           "ccl_set_profile_events", "ccl_set_tuning", "ccl_last_error",
+           "ccl_set_profile_events", "ccl_set_option", "ccl_last_error",
            "ccl_version", "ccl_launch_count"]
 
 _vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
@@ -33,7 +33,7 @@ lib.ccl_version.argtypes = []
 lib.ccl_launch_count.restype = _i64
 lib.ccl_launch_count.argtypes = []
 lib.ccl_set_profile_events.argtypes = [_vp, _vp, _vp]
-lib.ccl_set_tuning.argtypes = [_i64, _i32, _i32, _i64]
+lib.ccl_set_option.argtypes = [C.c_char_p, _i64]
 for _n in EXPORTS[:11]:
     getattr(lib, _n).restype = C.c_int
 
@@ -120,9 +120,18 @@ def set_profile_events(after_init=None, after_reduce=None, after_flatten=None):
     _check(lib.ccl_set_profile_events(h(after_init), h(after_reduce), h(after_flatten)), "ccl_set_profile_events")
 
 
+def set_option(name, value=0):
+    """ccl_set_option(name, value); see include/ccl.h for the names."""
+    _check(lib.ccl_set_option(name.encode(), int(value)), "ccl_set_option")
+
+
 def set_tuning(bucket_min_label_bytes=-1, region_shift=-1, force_mode=-1, bucket_capacity=0):
-    """ccl_set_tuning; the defaults restore the library defaults."""
-    _check(lib.ccl_set_tuning(bucket_min_label_bytes, region_shift, force_mode, bucket_capacity), "ccl_set_tuning")
+    """Convenience for the tests: reset, then set the four knobs of the bucketed form."""
+    set_option("reset")
+    set_option("bucket_min_label_bytes", bucket_min_label_bytes)
+    set_option("region_shift", region_shift)
+    set_option("force_mode", force_mode)
+    set_option("bucket_capacity", bucket_capacity)
 
 
 def validate_bonds(n_sites, src, dst):

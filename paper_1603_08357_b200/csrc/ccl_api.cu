@@ -53,23 +53,34 @@ extern "C" const char* ccl_last_error(void) { return ccl::g_error; }
 extern "C" int ccl_version(void) { return 100; }      // 0.1.0
 extern "C" int64_t ccl_launch_count(void) { return ccl::g_launches; }
 
-extern "C" int ccl_set_tuning(int64_t bucket_min_label_bytes, int32_t region_shift, int32_t force_mode,
-                              int64_t bucket_capacity)
+extern "C" int ccl_set_option(const char* name, int64_t value)
 {
     ccl::Tuning def;
     ccl::Tuning& t = ccl::tuning();
-    if (region_shift >= 0 && (region_shift < 4 || region_shift > 30)) {
-        ccl::set_error("invalid argument: region_shift must lie in [4, 30]");
-        return CCL_INVALID_ARG;
+    if (name == nullptr) { ccl::set_error("invalid argument: option name is NULL"); return CCL_INVALID_ARG; }
+    if (!strcmp(name, "reset")) { t = def; return CCL_OK; }
+    if (!strcmp(name, "bucket_min_label_bytes")) {
+        t.bucket_min_label_bytes = value >= 0 ? value : def.bucket_min_label_bytes;
+        t.bucket_min_bonds = value >= 0 ? 0 : def.bucket_min_bonds;
+        return CCL_OK;
     }
-    if (force_mode < -1 || force_mode > 1) {
-        ccl::set_error("invalid argument: force_mode must be -1, 0 or 1");
-        return CCL_INVALID_ARG;
+    if (!strcmp(name, "region_shift")) {
+        if (value >= 0 && (value < 4 || value > 30)) {
+            ccl::set_error("invalid argument: region_shift must lie in [4, 30]");
+            return CCL_INVALID_ARG;
+        }
+        t.region_shift = value >= 0 ? (int32_t)value : def.region_shift;
+        return CCL_OK;
     }
-    t.bucket_min_label_bytes = bucket_min_label_bytes >= 0 ? bucket_min_label_bytes : def.bucket_min_label_bytes;
-    t.bucket_min_bonds = bucket_min_label_bytes >= 0 ? 0 : def.bucket_min_bonds;
-    t.region_shift = region_shift >= 0 ? region_shift : def.region_shift;
-    t.force_mode = force_mode;
-    t.bucket_capacity = bucket_capacity > 0 ? bucket_capacity : 0;
-    return CCL_OK;
+    if (!strcmp(name, "force_mode")) {
+        if (value < -1 || value > 1) {
+            ccl::set_error("invalid argument: force_mode must be -1, 0 or 1");
+            return CCL_INVALID_ARG;
+        }
+        t.force_mode = (int32_t)value;
+        return CCL_OK;
+    }
+    if (!strcmp(name, "bucket_capacity")) { t.bucket_capacity = value > 0 ? value : 0; return CCL_OK; }
+    ccl::set_error("invalid argument: unknown option '%s'", name);
+    return CCL_INVALID_ARG;
 }

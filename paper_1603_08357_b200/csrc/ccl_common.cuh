@@ -57,7 +57,7 @@ struct BucketHeader {                              // lives in device memory at 
                                                    // excess was joined on the spot by the general algorithm)
 };
 
-struct Tuning {                                    // ccl_set_tuning(); process-wide
+struct Tuning {                                    // ccl_set_option(); process-wide
     int64_t bucket_min_label_bytes = 96ll << 20;   // label[] beyond this cannot stay resident in the 126 MB L2
     int64_t bucket_min_bonds = 1 << 20;
     int32_t region_shift = 23;                     // 2^23 sites = 32 MiB of labels per region
@@ -111,12 +111,16 @@ __device__ __forceinline__ uint32_t ld_stream_u8(const uint8_t* p, uint64_t pol)
     return r;
 }
 
-// Label reads during root finding.  Relaxed, L2-coherent (bypasses the non-coherent L1): a stale value would
-// still be a valid ancestor, but fresh values shorten the walks.
+// Label reads during root finding and flattening go through L1 (ld.global.ca).  L1 is not coherent, so a read may
+// return an older value of label[x] -- which is still an ancestor of x, so every walk stays correct and only gets a
+// little longer; every decision that matters is re-validated by the value an atomicMin
+// returns.  What L1 buys: the top of a big cluster's tree is read by every walk through that cluster, and with
+// L2-only loads (ld.relaxed.gpu, the first version) those reads all queue up at the one L2 slice that owns the
+// sector (profiles/r1_notes.md).
 __device__ __forceinline__ int32_t ld_label(const int32_t* p)
 {
     int32_t r;
-    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(r) : "l"(p) : "memory");
+    asm volatile("ld.global.ca.s32 %0, [%1];" : "=r"(r) : "l"(p) : "memory");
     return r;
 }
 __device__ __forceinline__ void st_label(int32_t* p, int32_t v)

@@ -33,10 +33,13 @@ __global__ void __launch_bounds__(kThreads) k_init(int64_t n_sites, int32_t* __r
 // MASK: 0 = every bond occupied, 1 = uint8 per bond, 2 = packed bits.  VEC: src/dst 16-byte aligned (and the
 // uint8 mask 4-byte aligned), so a thread fetches its 4 bonds with two 128-bit loads.
 template <int MASK, bool VEC>
-__device__ __forceinline__ void reduce4(int64_t n_bonds, int64_t b0, const int32_t* __restrict__ src,
-                                        const int32_t* __restrict__ dst, const void* __restrict__ occ,
-                                        int32_t* label, uint64_t pol)
+__device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_t* __restrict__ src,
+                                       const int32_t* __restrict__ dst, const void* __restrict__ occ,
+                                       int32_t* label, uint64_t pol, int32_t (&pa)[4], int32_t (&pb)[4])
 {
+    // Loads this thread's (up to) 4 bonds, does the first-touch atomics, and returns how many pairs are left to join;
+    // they are stored in pa[]/pb[] front-packed.
+    if (b0 >= n_bonds) return 0;
     const int cnt = (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
 
     // occupancy of this thread's 4 bonds -> low 4 bits of m
@@ -55,7 +58,7 @@ __device__ __forceinline__ void reduce4(int64_t n_bonds, int64_t b0, const int32
         }
     }
     m &= (1u << cnt) - 1u;
-    if (m == 0) return;
+    if (m == 0) return 0;
 
     int32_t u[4], v[4];
     if (VEC && cnt == 4) {
@@ -84,21 +87,54 @@ __device__ __forceinline__ void reduce4(int64_t n_bonds, int64_t b0, const int32
             old[k] = (o == hi) ? lo[k] : o;
         }
     }
+    int n = 0;
 #pragma unroll
     for (int k = 0; k < 4; ++k)
-        if (old[k] != lo[k]) algorithm1(label, old[k], lo[k]);
+        if (old[k] != lo[k]) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) if (q == n) { pa[q] = old[k]; pb[q] = lo[k]; }    // keeps pa/pb in registers
+            ++n;
+        }
+    return n;
 }
 
+// One pass over the bond stream.  About a quarter of the occupied bonds survive the first touch and need root
+// walks, which are long chains of dependent L2 loads; left where they arise they would keep a quarter of the lanes
+// busy for four rounds.  So every warp packs its survivors into a shared-memory queue and then works through the
+// queue with all lanes.
 template <int MASK, bool VEC>
 __global__ void __launch_bounds__(kThreads)
 k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
          const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr)
 {
+    __shared__ int2 queue[kThreads / 32][128];
     if (hdr != nullptr && hdr->mode == 1) return;          // the bucketed form (ccl_bucket.cu) did step (iii)
     const uint64_t pol = evict_first_policy();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
-    for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_bonds; b0 += stride)
-        reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol);
+    const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
+    for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
+        int32_t pa[4], pb[4];
+        const int n = reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol, pa, pb);
+        int incl = n;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        if (total == 0) continue;
+        const int off = incl - n;
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (q < n) queue[warp][off + q] = make_int2(pa[q], pb[q]);
+        __syncwarp();
+        for (int j = lane; j < total; j += 32) {
+            const int2 pr = queue[warp][j];
+            algorithm1(label, pr.x, pr.y);
+        }
+        __syncwarp();
+    }
 }
 
 // ----------------------------------------------------------------------------------------------- step (iv)
@@ -115,15 +151,23 @@ __global__ void __launch_bounds__(kThreads) k_flatten(int64_t n_sites, int32_t* 
         int32_t par[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) par[k] = (cur[k] == (int32_t)(i0 + k)) ? cur[k] : ld_label(label + cur[k]);
-        bool changed = false;
+        // the four chases advance together: one round = up to four independent loads in flight
+        int32_t c[4] = {cur[0], cur[1], cur[2], cur[3]};
+        for (;;) {
+            bool w[4], any = false;
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            int32_t c = cur[k], p = par[k];
-            while (p != c) { c = p; p = ld_label(label + c); }
-            changed |= (c != cur[k]);
-            cur[k] = c;
+            for (int k = 0; k < 4; ++k) { w[k] = par[k] != c[k]; any |= w[k]; }
+            if (!any) break;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) if (w[k]) c[k] = par[k];
+            int32_t nx[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) nx[k] = w[k] ? ld_label(label + c[k]) : par[k];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) par[k] = nx[k];
         }
-        if (changed) *reinterpret_cast<int4*>(label + i0) = make_int4(cur[0], cur[1], cur[2], cur[3]);
+        const bool changed = (c[0] != cur[0]) | (c[1] != cur[1]) | (c[2] != cur[2]) | (c[3] != cur[3]);
+        if (changed) *reinterpret_cast<int4*>(label + i0) = make_int4(c[0], c[1], c[2], c[3]);
     } else {
         for (int64_t i = i0; i < n_sites; ++i) {
             int32_t c = label[i], p = ld_label(label + c);

@@ -23,12 +23,37 @@ __device__ __forceinline__ int32_t find_root(int32_t* label, int32_t x)
     return x;
 }
 
+// The two root walks of Algorithm 1 advanced together: both chains issue their loads in the same
+// step, so the dependent-load depth is the longer of the two walks instead of their sum.  Same path halving.
+__device__ __forceinline__ void find_roots2(int32_t* label, int32_t& a, int32_t& b)
+{
+    int32_t pa = ld_label(label + a), pb = ld_label(label + b);        // invariant: pa = a value read from label[a]
+    for (;;) {
+        const bool wa = pa != a, wb = pb != b;                         // still walking?
+        if (!wa && !wb) return;
+        const int32_t ga = wa ? ld_label(label + pa) : pa;             // grandparents, both loads in flight together
+        const int32_t gb = wb ? ld_label(label + pb) : pb;
+        bool la = false, lb = false;
+        if (wa) {
+            if (ga == pa) a = pa;                                      // pa is a root (and pa == a now)
+            else { st_label(label + a, ga); a = ga; la = true; }       // halve: a -> grandparent, move there
+        }
+        if (wb) {
+            if (gb == pb) b = pb;
+            else { st_label(label + b, gb); b = gb; lb = true; }
+        }
+        const int32_t na = la ? ld_label(label + a) : pa;
+        const int32_t nb = lb ? ld_label(label + b) : pb;
+        pa = na; pb = nb;
+    }
+}
+
 // Algorithm 1 (reading R3 of its garbled last lines, exit test R4): make sure sites a and b end
 // up in one tree.  label_1 is the larger of the two current representatives, label_2 the smaller.
 __device__ __forceinline__ void algorithm1(int32_t* label, int32_t a, int32_t b)
 {
-    int32_t label_1 = find_root(label, a);
-    int32_t label_2 = find_root(label, b);
+    int32_t label_1 = a, label_2 = b;
+    find_roots2(label, label_1, label_2);
     while (label_1 != label_2) {
         if (label_1 < label_2) { const int32_t t = label_1; label_1 = label_2; label_2 = t; }
         const int32_t label_3 = atomicMin(label + label_1, label_2);
@@ -37,8 +62,8 @@ __device__ __forceinline__ void algorithm1(int32_t* label, int32_t a, int32_t b)
         // replaced by label_1 -> label_2, so label_3 must be joined to label_2; if label_3 < label_2 nothing was
         // written and label_1 hangs under label_3, which must be joined to label_2.  Either way the pair to join
         // is (label_3, label_2); walk both up to their roots before the next atomic.
-        label_1 = find_root(label, label_3);
-        label_2 = find_root(label, label_2);
+        label_1 = label_3;
+        find_roots2(label, label_1, label_2);
     }
 }
 
