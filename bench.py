@@ -153,6 +153,27 @@ def cpu_oracle_sample(name, steps, warmup):
     return len(ps) * src.size / per_step / 1e9, per_step, sample
 
 
+def replica_plan(rank, cfg):
+    """Replicas only: every rank labels its own realization of the same workload."""
+    return {"seed": SEED_BASE + cfg, "realization": rank}
+
+
+def max_over_ranks(value, world, device="cpu"):
+    """MAX over ranks of a host scalar (device timing): one all-reduce of the timing scalar, nothing on the data path."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world, calls_per_step, n_bonds, ms_per_step):
+    """Whole-job Gbonds/s: every rank processes calls_per_step * n_bonds bonds per step, in the slowest rank's time."""
+    return world * calls_per_step * n_bonds / (ms_per_step * 1e-3) / 1e9
+
+
 def run_reference(args):
     """--impl reference: the oracle timed on the host cores (this tier has no other reference implementation)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -206,8 +227,10 @@ def run_ours(args):
     else:
         src, dst = ccl.gen_triangular(size)
     masks = []
+    plan = replica_plan(rank, cfg)
     for p in ps:                      # replicas differ by realization = rank
-        mask, bits = ccl.gen_occupancy(m, p, seed, rank, want_mask=(kind == "u8"), want_bits=(kind != "u8"))
+        mask, bits = ccl.gen_occupancy(m, p, plan["seed"], plan["realization"], want_mask=(kind == "u8"),
+                                       want_bits=(kind != "u8"))
         masks.append(mask if kind == "u8" else bits)
     labels = torch.empty(n, dtype=torch.int32, device="cuda")
     torch.cuda.synchronize()
@@ -268,12 +291,9 @@ def run_ours(args):
     flat_ms = [e[2].elapsed_time(e[3]) for e in ev]
     if flush is not None:
         total_ms = sum(call_ms)                       # exclude the flush writes from the step time
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, "cuda")
     ms_per_step = total_ms / K
-    value = world * len(ps) * m / (ms_per_step * 1e-3) / 1e9
+    value = job_value(world, len(ps), m, ms_per_step)
 
     peak, peak_src = measured_peak()
     avg = lambda xs: sum(xs) / len(xs)
@@ -311,10 +331,7 @@ def run_ours(args):
                 ccl.label_bits_host(n, hs, hd, hm[k], hl)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, world, "cuda")
         h2d = len(ps) * (2 * 4 * m + 4 * ((m + 31) // 32))
         d2h = len(ps) * 4 * n
         e2e = {"value": world * len(ps) * m * e2e_steps / dt / 1e9, "unit": "Gbonds/s", "h2d_bytes_per_step": h2d,
