@@ -46,5 +46,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_ubench() -> str:
+    """The random-access microbenchmark of DESIGN.md section 6 (standalone executable, not part of libccl.so)."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    out = os.path.join(HERE, "ccl_ubench.bin")
+    subprocess.check_call([nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-o", out,
+                           os.path.join(CSRC, "ccl_ubench.cu")])
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force=True, verbose="-v" in sys.argv))
+    if "--ubench" in sys.argv:
+        print(build_ubench())
+    else:
+        print(build(force=True, verbose="-v" in sys.argv))
