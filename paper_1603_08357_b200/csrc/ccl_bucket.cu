@@ -38,7 +38,8 @@ template <int P>
 struct EmitSmem {
     int cnt[kMaxRegions];
     int pref[kMaxRegions + 1];
-    unsigned long long base[kMaxRegions];
+    int lim[kMaxRegions];                 // staging indices below lim[r] fit into bucket r
+    int2* gptr[kMaxRegions];              // bucket r's slot of staging index j is gptr[r] + j
     int2 stage[kBThreads * P];
 };
 
@@ -63,9 +64,13 @@ __device__ __forceinline__ void cta_emit(EmitSmem<P>& sm, const int32_t (&lo)[P]
             const int t = __shfl_up_sync(0xffffffffu, incl, o);
             if (tid >= o) incl += t;
         }
-        sm.pref[tid] = incl - c;
+        const int pref = incl - c;
+        sm.pref[tid] = pref;
         if (tid == 31) sm.pref[32] = incl;
-        sm.base[tid] = c ? atomicAdd(&hdr->count[tid], (unsigned long long)c) : 0ull;
+        const unsigned long long base = c ? atomicAdd(&hdr->count[tid], (unsigned long long)c) : 0ull;
+        const unsigned long long room = base < cap ? cap - base : 0ull;          // free slots left in bucket tid
+        sm.lim[tid] = pref + (int)(room < (unsigned long long)c ? room : (unsigned long long)c);
+        sm.gptr[tid] = buckets + (size_t)tid * cap + base - pref;
     }
     __syncthreads();
 #pragma unroll
@@ -76,8 +81,7 @@ __device__ __forceinline__ void cta_emit(EmitSmem<P>& sm, const int32_t (&lo)[P]
     for (int j = tid; j < total; j += kBThreads) {
         const int2 pr = sm.stage[j];
         const int r = pr.y >> shift;
-        const unsigned long long pos = sm.base[r] + (unsigned long long)(j - sm.pref[r]);
-        if (pos < cap) st_stream_pair(buckets + (size_t)r * cap + pos, pr, pol);
+        if (j < sm.lim[r]) st_stream_pair(sm.gptr[r] + j, pr, pol);
         else algorithm1(label, pr.x, pr.y);          // bucket full: join the pair right here, the slow general way
     }
     __syncthreads();
@@ -160,10 +164,10 @@ k_scatter(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __res
 
 // -------------------------------------------------------------------------------------------------- descend
 // Reduce region r: all label[] traffic of this launch falls into [r << shift, (r+1) << shift).
+template <int P>
 __global__ void __launch_bounds__(kBThreads)
 k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long cap, int32_t* label)
 {
-    constexpr int P = 4;
     __shared__ EmitSmem<P> sm;
     if (hdr->mode != 1) return;
     const uint64_t pol = evict_first_policy();
@@ -175,9 +179,11 @@ k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long
         const unsigned long long i0 = ((unsigned long long)tile * kBThreads + threadIdx.x) * P;
         int32_t a[P], b[P], old[P];
         if (i0 + P <= n) {
-            const int4 q0 = ld_stream_v4(reinterpret_cast<const int32_t*>(bucket + i0), pol);
-            const int4 q1 = ld_stream_v4(reinterpret_cast<const int32_t*>(bucket + i0 + 2), pol);
-            a[0] = q0.x; b[0] = q0.y; a[1] = q0.z; b[1] = q0.w; a[2] = q1.x; b[2] = q1.y; a[3] = q1.z; b[3] = q1.w;
+#pragma unroll
+            for (int q = 0; q < P / 2; ++q) {
+                const int4 v = ld_stream_v4(reinterpret_cast<const int32_t*>(bucket + i0 + 2 * q), pol);
+                a[2 * q] = v.x; b[2 * q] = v.y; a[2 * q + 1] = v.z; b[2 * q + 1] = v.w;
+            }
         } else {
 #pragma unroll
             for (int k = 0; k < P; ++k) {
@@ -223,7 +229,7 @@ int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const 
     const int n_regions = (int)(((n_sites - 1) >> shift) + 1);
     unsigned long long cap = (unsigned long long)((4 * n_bonds) / n_regions + 4096);
     if (tuning().bucket_capacity > 0) cap = (unsigned long long)tuning().bucket_capacity;
-    cap = (cap + 3ull) & ~3ull;                                   // keeps every bucket 32-byte aligned
+    cap = (cap + 7ull) & ~7ull;                                   // keeps every bucket 64-byte aligned
     const size_t hdr_bytes = (sizeof(BucketHeader) + 255) & ~(size_t)255;
     const size_t bytes = hdr_bytes + (size_t)n_regions * cap * sizeof(int2);
     void* ws = nullptr;
@@ -246,7 +252,7 @@ int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const 
         k_scatter<2><<<grid, kBThreads, 0, st>>>(n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels);
     CCL_CHECK_LAUNCH("k_scatter");
     for (int r = n_regions - 1; r >= 0; --r) {
-        k_descend<<<grid, kBThreads, 0, st>>>(r, shift, hdr, buckets, cap, labels);
+        k_descend<4><<<grid, kBThreads, 0, st>>>(r, shift, hdr, buckets, cap, labels);
         CCL_CHECK_LAUNCH("k_descend");
     }
     return CCL_OK;
