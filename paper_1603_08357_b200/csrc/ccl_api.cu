@@ -81,6 +81,25 @@ extern "C" int ccl_set_option(const char* name, int64_t value)
         return CCL_OK;
     }
     if (!strcmp(name, "bucket_capacity")) { t.bucket_capacity = value > 0 ? value : 0; return CCL_OK; }
+    if (!strcmp(name, "tile_mode")) {
+        if (value < -1 || value > 1) {
+            ccl::set_error("invalid argument: tile_mode must be -1, 0 or 1");
+            return CCL_INVALID_ARG;
+        }
+        t.tile_mode = (int32_t)value;
+        return CCL_OK;
+    }
+    if (!strcmp(name, "sub_shift")) {
+        if (value > 15) {
+            ccl::set_error("invalid argument: sub_shift must be at most 15 (128 KiB of labels in shared memory)");
+            return CCL_INVALID_ARG;
+        }
+        t.sub_shift = value >= 2 ? (int32_t)value : -1;
+        return CCL_OK;
+    }
+    if (!strcmp(name, "fine_capacity")) { t.fine_capacity = value > 0 ? value : 0; return CCL_OK; }
+    if (!strcmp(name, "small_max_sites")) { t.small_max_sites = value >= 0 ? value : def.small_max_sites; return CCL_OK; }
+    if (!strcmp(name, "tile_min_bonds")) { t.tile_min_bonds = value >= 0 ? value : def.tile_min_bonds; return CCL_OK; }
     ccl::set_error("invalid argument: unknown option '%s'", name);
     return CCL_INVALID_ARG;
 }

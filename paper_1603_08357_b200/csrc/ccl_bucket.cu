@@ -20,81 +20,24 @@
 // (raster-ordered lattices) keep the direct one-pass kernel of ccl_label.cu, whose gathers hit L2 anyway.
 #include "ccl_common.cuh"
 #include "ccl_unionfind.cuh"
+#include "ccl_emit.cuh"
 
 namespace ccl {
 
 constexpr int kBThreads = 256;
-
-__device__ __forceinline__ void st_stream_pair(int2* p, int2 v, uint64_t pol)
-{
-    asm volatile("st.global.L2::cache_hint.v2.s32 [%0], {%1, %2}, %3;" ::"l"(p), "r"(v.x), "r"(v.y), "l"(pol)
-                 : "memory");
-}
-
-// Shared-memory scratch of the CTA-wide append: pairs are counted per target region, one global atomicAdd per
-// region reserves the CTA's range in that bucket, and the pairs leave through a staging array so that consecutive
-// threads write consecutive addresses.
-template <int P>
-struct EmitSmem {
-    int cnt[kMaxRegions];
-    int pref[kMaxRegions + 1];
-    int lim[kMaxRegions];                 // staging indices below lim[r] fit into bucket r
-    int2* gptr[kMaxRegions];              // bucket r's slot of staging index j is gptr[r] + j
-    int2 stage[kBThreads * P];
-};
-
-// Every thread hands in up to P pairs (lo[k] < 0 = none).  Must be called by all threads of the CTA.
-template <int P>
-__device__ __forceinline__ void cta_emit(EmitSmem<P>& sm, const int32_t (&lo)[P], const int32_t (&hi)[P], int shift,
-                                         BucketHeader* hdr, int2* buckets, unsigned long long cap, int32_t* label,
-                                         uint64_t pol)
-{
-    const int tid = threadIdx.x;
-    if (tid < kMaxRegions) sm.cnt[tid] = 0;
-    __syncthreads();
-    int rank[P];
-#pragma unroll
-    for (int k = 0; k < P; ++k) rank[k] = (lo[k] >= 0) ? atomicAdd(&sm.cnt[hi[k] >> shift], 1) : 0;
-    __syncthreads();
-    if (tid < 32) {
-        const int c = sm.cnt[tid];
-        int incl = c;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, incl, o);
-            if (tid >= o) incl += t;
-        }
-        const int pref = incl - c;
-        sm.pref[tid] = pref;
-        if (tid == 31) sm.pref[32] = incl;
-        const unsigned long long base = c ? atomicAdd(&hdr->count[tid], (unsigned long long)c) : 0ull;
-        const unsigned long long room = base < cap ? cap - base : 0ull;          // free slots left in bucket tid
-        sm.lim[tid] = pref + (int)(room < (unsigned long long)c ? room : (unsigned long long)c);
-        sm.gptr[tid] = buckets + (size_t)tid * cap + base - pref;
-    }
-    __syncthreads();
-#pragma unroll
-    for (int k = 0; k < P; ++k)
-        if (lo[k] >= 0) sm.stage[sm.pref[hi[k] >> shift] + rank[k]] = make_int2(lo[k], hi[k]);
-    __syncthreads();
-    const int total = sm.pref[32];
-    for (int j = tid; j < total; j += kBThreads) {
-        const int2 pr = sm.stage[j];
-        const int r = pr.y >> shift;
-        if (j < sm.lim[r]) st_stream_pair(sm.gptr[r] + j, pr, pol);
-        else algorithm1(label, pr.x, pr.y);          // bucket full: join the pair right here, the slow general way
-    }
-    __syncthreads();
-}
 
 // ---------------------------------------------------------------------------------------------------- probe
 // Samples bonds at a fixed stride and looks at how many join two different regions.  Random numbering: 1 - 1/R of
 // them; raster-ordered lattice: only those on region borders.
 __global__ void __launch_bounds__(1024)
 k_probe(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, int shift, int force_mode,
-        BucketHeader* hdr)
+        const int32_t* gate, BucketHeader* hdr)
 {
     __shared__ int s_cross;
+    if (gate != nullptr && *gate == 0) {               // the tiled form (ccl_tile.cu) has done steps (i)-(iii)
+        if (threadIdx.x == 0) hdr->mode = 2;
+        return;
+    }
     if (threadIdx.x == 0) s_cross = 0;
     __syncthreads();
     const int64_t samples = n_bonds < 8192 ? n_bonds : 8192;
@@ -119,7 +62,7 @@ k_scatter(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __res
           unsigned long long cap, int32_t* label)
 {
     constexpr int P = 8;
-    __shared__ EmitSmem<P> sm;
+    __shared__ EmitSmem<kBThreads, P> sm;
     if (hdr->mode != 1) return;
     const uint64_t pol = evict_first_policy();
     const int64_t tiles = (n_bonds + kBThreads * P - 1) / (kBThreads * P);
@@ -158,7 +101,7 @@ k_scatter(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __res
             lo[k] = on ? min(u[k], v[k]) : -1;
             hi[k] = max(u[k], v[k]);
         }
-        cta_emit<P>(sm, lo, hi, shift, hdr, buckets, cap, label, pol);
+        cta_emit<kBThreads, P>(sm, lo, hi, shift, hdr, buckets, cap, JoinNow{label}, pol);
     }
 }
 
@@ -168,7 +111,7 @@ template <int P>
 __global__ void __launch_bounds__(kBThreads)
 k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long cap, int32_t* label)
 {
-    __shared__ EmitSmem<P> sm;
+    __shared__ EmitSmem<kBThreads, P> sm;
     if (hdr->mode != 1) return;
     const uint64_t pol = evict_first_policy();
     unsigned long long n = hdr->count[r];
@@ -215,13 +158,14 @@ k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long
             a[k] = pending ? aa : -1;
             b[k] = bb;
         }
-        cta_emit<P>(sm, a, b, shift, hdr, buckets, cap, label, pol);
+        cta_emit<kBThreads, P>(sm, a, b, shift, hdr, buckets, cap, JoinNow{label}, pol);
     }
 }
 
 // ------------------------------------------------------------------------------------------------- host side
 int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                    int mask_kind, int32_t* labels, cudaStream_t st, BucketHeader** hdr_out, void** ws_out)
+                    int mask_kind, int32_t* labels, cudaStream_t st, const int32_t* gate, BucketHeader** hdr_out,
+                    void** ws_out)
 {
     // region size: 2^23 sites (32 MiB of labels) unless that would need more than kMaxRegions regions
     int shift = tuning().region_shift;
@@ -239,7 +183,7 @@ int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const 
     int2* buckets = reinterpret_cast<int2*>(static_cast<char*>(ws) + hdr_bytes);
     *hdr_out = hdr;
     CCL_CUDA_TRY(cudaMemsetAsync(hdr, 0, sizeof(BucketHeader), st));
-    k_probe<<<1, 1024, 0, st>>>(n_bonds, src, dst, shift, tuning().force_mode, hdr);
+    k_probe<<<1, 1024, 0, st>>>(n_bonds, src, dst, shift, tuning().force_mode, gate, hdr);
     CCL_CHECK_LAUNCH("k_probe");
     const uintptr_t al = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     const int vec = (al & 15) == 0;

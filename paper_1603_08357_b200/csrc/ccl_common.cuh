@@ -57,12 +57,29 @@ struct BucketHeader {                              // lives in device memory at 
                                                    // excess was joined on the spot by the general algorithm)
 };
 
+// Header of the tiled form's workspace (ccl_tile.cu).  Starts with a BucketHeader so that k_descend and cta_emit work
+// on the region buckets unchanged.
+constexpr int kMaxSubRegions = 2048;               // sub-regions (tiles of label[] held in shared memory) per call
+constexpr int kFineStride = 8;                     // one fine counter per 32-byte sector (no false sharing in L2)
+struct TileHeader {
+    BucketHeader bh;
+    unsigned long long overflow;                   // pairs in the overflow list
+    unsigned long long pad;
+    unsigned int fine[kMaxSubRegions * kFineStride];   // pairs filed under sub-region s: fine[s * kFineStride]
+};
+
 struct Tuning {                                    // ccl_set_option(); process-wide
     int64_t bucket_min_label_bytes = 96ll << 20;   // label[] beyond this cannot stay resident in the 126 MB L2
     int64_t bucket_min_bonds = 1 << 20;
     int32_t region_shift = 23;                     // 2^23 sites = 32 MiB of labels per region
     int32_t force_mode = -1;                       // -1: device-side probe decides; 0: direct; 1: bucketed
     int64_t bucket_capacity = 0;                   // pairs per region bucket; 0 = 4 M / regions + 4096
+    int32_t tile_mode = 0;                         // tiled form (ccl_tile.cu): 0 off (default: measured slower, see
+                                                   // profiles/r1_notes.md), -1 a device-side probe decides, 1 always
+    int32_t sub_shift = -1;                        // 2^sub_shift sites per sub-region; -1 = from n_sites
+    int64_t fine_capacity = 0;                     // pairs per sub-region bucket; 0 = 2 M / S + 8192
+    int64_t tile_min_bonds = 1 << 18;
+    int64_t small_max_sites = 1 << 15;             // one-CTA kernel for label arrays up to this many sites              // auto: calls with fewer bonds keep the direct kernel
 };
 Tuning& tuning();
 
@@ -72,8 +89,20 @@ int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st);
 
 // Enqueues probe + scatter + one descend launch per region.  *ws_out is a cudaMallocAsync allocation the caller
 // frees (cudaFreeAsync) after the kernels that read *hdr_out have been enqueued.
+// gate (may be NULL): device flag; if *gate == 0 the tiled form has done the work and the probe sets mode 2 (nothing).
 int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                    int mask_kind, int32_t* labels, cudaStream_t st, BucketHeader** hdr_out, void** ws_out);
+                    int mask_kind, int32_t* labels, cudaStream_t st, const int32_t* gate, BucketHeader** hdr_out,
+                    void** ws_out);
+
+// Tiled form of steps (i)-(iii) for bond lists that are local in the site numbering (ccl_tile.cu).  *done says what
+// was enqueued: kTiledNo nothing (call outside its range); kTiledFinal labels are final (one-CTA kernel); kTiledIfLocal
+// a device-side probe decides -- *not_local points at a device flag that is 0 if the tiled kernels did steps (i)-(iii)
+// and non-zero if they returned at once, so the caller enqueues the other forms gated on it; kTiledForced the tiled
+// kernels ran unconditionally.  *ws_out (if set) is freed by the caller with cudaFreeAsync after the last kernel that
+// reads the flag has been enqueued.
+enum { kTiledNo = 0, kTiledFinal = 1, kTiledIfLocal = 2, kTiledForced = 3 };
+int tiled_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
+                 int mask_kind, int32_t* labels, cudaStream_t st, int* done, const int32_t** not_local, void** ws_out);
 
 // ---- device helpers --------------------------------------------------------------------------------------
 // Streaming (read-once) loads: bypass L1 allocation and mark the L2 line evict-first, so that the bond stream

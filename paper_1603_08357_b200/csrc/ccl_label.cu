@@ -16,8 +16,9 @@ namespace ccl {
 constexpr int kThreads = 256;
 
 // ------------------------------------------------------------------------------------------------ step (i)
-__global__ void __launch_bounds__(kThreads) k_init(int64_t n_sites, int32_t* __restrict__ label)
+__global__ void __launch_bounds__(kThreads) k_init(int64_t n_sites, int32_t* __restrict__ label, const int32_t* gate)
 {
+    if (gate != nullptr && *gate == 0) return;             // the tiled form (ccl_tile.cu) has written every label
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
     for (int64_t i = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; i < n_sites; i += stride) {
         if (i + 4 <= n_sites) {
@@ -105,10 +106,11 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
 template <int MASK, bool VEC>
 __global__ void __launch_bounds__(kThreads)
 k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr)
+         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
 {
     __shared__ int2 queue[kThreads / 32][128];
-    if (hdr != nullptr && hdr->mode == 1) return;          // the bucketed form (ccl_bucket.cu) did step (iii)
+    if (hdr != nullptr && hdr->mode != 0) return;          // the bucketed form (ccl_bucket.cu) did step (iii)
+    if (gate != nullptr && *gate == 0) return;             // the tiled form (ccl_tile.cu) did
     const uint64_t pol = evict_first_policy();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
@@ -206,11 +208,11 @@ static int check_args(int64_t n_sites, int64_t n_bonds, const void* src, const v
 
 template <int MASK>
 static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                         int32_t* labels, const BucketHeader* hdr, cudaStream_t st)
+                         int32_t* labels, const BucketHeader* hdr, const int32_t* gate, cudaStream_t st)
 {
     const int64_t groups = (n_bonds + 3) / 4;
     int64_t blocks = (groups + kThreads - 1) / kThreads;
-    if (blocks > (int64_t)kSMs * 8 * 16) blocks = (int64_t)kSMs * 8 * 16;     // grid-stride beyond 16 waves of 8 CTAs/SM
+    if (blocks > (int64_t)kSMs * 8 * 4) blocks = (int64_t)kSMs * 8 * 4;       // grid-stride beyond 4 waves of 8 CTAs/SM
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     bool vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
@@ -218,8 +220,8 @@ static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst
         set_error("invalid argument: occupied_bits is not 4-byte aligned");
         return CCL_INVALID_ARG;
     }
-    if (vec) k_reduce<MASK, true><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels, hdr);
-    else     k_reduce<MASK, false><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels, hdr);
+    if (vec) k_reduce<MASK, true><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels, hdr, gate);
+    else     k_reduce<MASK, false><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels, hdr, gate);
     CCL_CHECK_LAUNCH("k_reduce");
     return CCL_OK;
 }
@@ -243,31 +245,46 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
     if (!lab_vec) { set_error("labels must be 16-byte aligned"); return CCL_UNSUPPORTED; }
 
     const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
-    const int64_t init_blocks = site_blocks < (int64_t)kSMs * 32 ? site_blocks : (int64_t)kSMs * 32;
-    k_init<<<(unsigned)init_blocks, kThreads, 0, st>>>(n_sites, labels);                      // step (i)
-    CCL_CHECK_LAUNCH("k_init");
+    // Tiled form (ccl_tile.cu): steps (i)-(iii) with the label reduction in shared memory, for bond lists that are local
+    // in the site numbering.  A device-side probe decides; the kernels of the other forms are enqueued behind it and
+    // return at once when it did the work (*gate == 0), so no decision ever needs a host round trip.
+    int tiled = kTiledNo;
+    const int32_t* gate = nullptr;
+    void* tile_ws = nullptr;
+    rc = tiled_reduce(n_sites, n_bonds, src, dst, occ, mask_kind, labels, st, &tiled, &gate, &tile_ws);
+    if (rc != CCL_OK) return rc;
+    auto done = [&](int code) { if (tile_ws) cudaFreeAsync(tile_ws, st); return code; };
+    if (tiled == kTiledFinal) { mark(0, st); mark(1, st); mark(2, st); return CCL_OK; }
+    if (tiled != kTiledForced) {
+        const int64_t init_blocks = site_blocks < (int64_t)kSMs * 32 ? site_blocks : (int64_t)kSMs * 32;
+        k_init<<<(unsigned)init_blocks, kThreads, 0, st>>>(n_sites, labels, gate);              // step (i)
+        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_init failed: %s", cudaGetErrorString(e)); return done(CCL_CUDA_ERROR); } count_launch(); }
+    }
     // step (ii): nothing to do after label[i] = i (every site is a root).
     mark(0, st);
     if (n_bonds > 0) {
-        // step (iii).  Label arrays that cannot stay in L2 get the region-bucketed form if a device-side probe finds
-        // the bonds non-local in the site numbering; the direct kernel then returns at once (and vice versa).
-        BucketHeader* hdr = nullptr;
-        void* ws = nullptr;
-        if (tuning().force_mode != 0 && n_sites * (int64_t)sizeof(int32_t) >= tuning().bucket_min_label_bytes &&
-            n_bonds >= tuning().bucket_min_bonds) {
-            rc = bucketed_reduce(n_sites, n_bonds, src, dst, occ, mask_kind, labels, st, &hdr, &ws);
-            if (rc != CCL_OK) { if (ws) cudaFreeAsync(ws, st); return rc; }
+        if (tiled != kTiledForced) {
+            // step (iii).  Label arrays that cannot stay in L2 get the region-bucketed form if a device-side probe finds
+            // the bonds non-local in the site numbering; the direct kernel then returns at once (and vice versa).
+            BucketHeader* hdr = nullptr;
+            void* ws = nullptr;
+            if (tuning().force_mode != 0 && n_sites * (int64_t)sizeof(int32_t) >= tuning().bucket_min_label_bytes &&
+                n_bonds >= tuning().bucket_min_bonds) {
+                rc = bucketed_reduce(n_sites, n_bonds, src, dst, occ, mask_kind, labels, st, gate, &hdr, &ws);
+                if (rc != CCL_OK) { if (ws) cudaFreeAsync(ws, st); return done(rc); }
+            }
+            if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, hdr, gate, st);
+            else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, hdr, gate, st);
+            else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, hdr, gate, st);
+            if (ws) cudaFreeAsync(ws, st);
+            if (rc != CCL_OK) return done(rc);
         }
-        if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, hdr, st);
-        else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, hdr, st);
-        else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, hdr, st);
-        if (ws) cudaFreeAsync(ws, st);
-        if (rc != CCL_OK) return rc;
         mark(1, st);
         k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels);                 // step (iv)
-        CCL_CHECK_LAUNCH("k_flatten");
+        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_flatten failed: %s", cudaGetErrorString(e)); return done(CCL_CUDA_ERROR); } count_launch(); }
         mark(2, st);
     }
+    if (tile_ws) cudaFreeAsync(tile_ws, st);
     return CCL_OK;
 }
 
