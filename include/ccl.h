@@ -113,6 +113,27 @@ int ccl_cluster_stats(int64_t n_sites, const int32_t* labels, int32_t* size_scra
 int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_src, const int32_t* host_dst,
                         const uint32_t* host_occupied_bits, int32_t* host_labels, void* stream);
 
+/* ---- many realizations of one small graph in one launch ---------------------------
+ *
+ * The same bond list (src, dst, n_bonds) under n_batch packed occupancy masks: realization r reads the mask at
+ * occupied_bits + r * mask_stride_words (bond b = bit (b & 31) of word (b >> 5); NULL = every bond occupied in every
+ * realization) and writes labels[r * n_sites .. (r+1) * n_sites).  One CTA per realization runs steps (i)-(iv) of
+ * PAPER.md:113 with the whole label array in shared memory, so n_sites <= 32768 (else CCL_UNSUPPORTED: call
+ * ccl_label_bits per realization).  Percolation studies average many independent realizations; a single
+ * call on a lattice this small is bound by launch latency.  Same result per realization as ccl_label_bits. */
+int ccl_label_batch(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+                    const uint32_t* occupied_bits, int64_t mask_stride_words, int32_t n_batch, int32_t* labels,
+                    void* stream);
+
+/* ---- sequential cluster numbers ("to assign the labels sequentially ...") -----------------
+ *
+ * labels: canonical labels (output of ccl_label*).  seq_labels[i] = number of clusters whose label is smaller than
+ * labels[i], i.e. clusters numbered 0..C-1 in ascending order of their smallest site; *n_clusters (device int64,
+ * optional) = C.  seq_labels may alias labels.  Call with workspace == NULL to obtain the required size in
+ * *workspace_bytes (host pointer), then again with a device workspace of at least that size. */
+int ccl_relabel_sequential(int64_t n_sites, const int32_t* labels, int32_t* seq_labels, int64_t* n_clusters,
+                           void* workspace, size_t* workspace_bytes, void* stream);
+
 /* ---- tuning --------------------------------------------------------------------------------------------
  *
  * ccl_set_option(name, value): process-wide knobs; none of them changes the result of ccl_label.  Step (iii) has two
@@ -125,6 +146,10 @@ int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_sr
  *   "force_mode"              -1 = the probe decides (default), 0 = always direct, 1 = always bucketed when eligible
  *   "bucket_capacity"         pairs each region's bucket can hold (<= 0: 4 M / regions + 4096); pairs that do not
  *                             fit are joined on the spot by the general algorithm
+ *   "tile_mode"               tiled form of step (iii) for bond lists that are local in the site numbering (window of
+ *                             labels in shared memory): 0 = off (default), -1 = a device-side probe
+ *                             decides, 1 = always; "sub_shift" (window = 2^value sites, <= 15), "fine_capacity",
+ *                             "tile_min_bonds", "small_max_sites" tune it
  *   "reset"                   all defaults (value ignored)
  * Unknown names -> CCL_INVALID_ARG. */
 int ccl_set_option(const char* name, int64_t value);

@@ -93,6 +93,16 @@ def stats(labels, n_dense=0):
     return d, hd, hl
 
 
+def relabel_sequential(labels):
+    """the min-site labels renumbered sequentially.  Cluster k (k = 0..C-1) is the one with the k-th
+    smallest label; returns (seq, C).  Written out from the definition: a site is a root iff labels[i] == i, and
+    seq[i] = number of roots below labels[i]."""
+    labels = np.asarray(labels, dtype=np.int64)
+    is_root = labels == np.arange(labels.size)
+    below = np.cumsum(is_root) - is_root          # roots strictly below each index
+    return below[labels].astype(np.int32), int(is_root.sum())
+
+
 def wrap(n_sites, src, dst, dx, dy, occupied=None):
     """(wrap_x, wrap_y): does some cluster hold a cycle with non-zero x / y winding (reading R7)."""
     src, dst = _bonds(src, dst)

@@ -14,7 +14,7 @@ lib = C.CDLL(_LIB_PATH)
 
 EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangular", "ccl_gen_honeycomb",
            "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
-           "ccl_set_profile_events", "ccl_set_option", "ccl_last_error",
+           "ccl_set_profile_events", "ccl_set_option", "ccl_label_batch", "ccl_relabel_sequential", "ccl_last_error",
            "ccl_version", "ccl_launch_count"]
 
 _vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
@@ -34,7 +34,9 @@ lib.ccl_launch_count.restype = _i64
 lib.ccl_launch_count.argtypes = []
 lib.ccl_set_profile_events.argtypes = [_vp, _vp, _vp]
 lib.ccl_set_option.argtypes = [C.c_char_p, _i64]
-for _n in EXPORTS[:11]:
+lib.ccl_label_batch.argtypes = [_i64, _i64, _vp, _vp, _vp, _i64, _i32, _vp, _vp]
+lib.ccl_relabel_sequential.argtypes = [_i64, _vp, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
+for _n in EXPORTS[:13]:
     getattr(lib, _n).restype = C.c_int
 
 
@@ -92,6 +94,32 @@ def label_bits(n_sites, src, dst, occupied_bits, labels=None, n_bonds=None):
                               _dev(occupied_bits, torch.int32, "occupied_bits"),
                               _dev(labels, torch.int32, "labels"), _stream()), "ccl_label_bits")
     return labels
+
+
+def label_batch(n_sites, src, dst, occupied_bits, n_batch, labels=None):
+    """ccl_label_batch: occupied_bits is an int32 tensor [n_batch, words >= ceil(n_bonds/32)] (or None); returns int32
+    labels [n_batch, n_sites].  One launch, one CTA per realization; n_sites <= 32768."""
+    if labels is None:
+        labels = torch.empty((n_batch, n_sites), dtype=torch.int32, device=src.device)
+    stride = 0 if occupied_bits is None else (occupied_bits.shape[1] if occupied_bits.dim() == 2 else occupied_bits.numel() // max(n_batch, 1))
+    _check(lib.ccl_label_batch(n_sites, src.numel(), _dev(src, torch.int32, "src"), _dev(dst, torch.int32, "dst"),
+                               _dev(occupied_bits, torch.int32, "occupied_bits"), stride, n_batch,
+                               _dev(labels, torch.int32, "labels"), _stream()), "ccl_label_batch")
+    return labels
+
+
+def relabel_sequential(labels, out=None):
+    """ccl_relabel_sequential: canonical labels -> (sequential labels 0..C-1, C)."""
+    n = labels.numel()
+    if out is None:
+        out = torch.empty_like(labels)
+    need = C.c_size_t(0)
+    _check(lib.ccl_relabel_sequential(n, None, None, None, None, C.byref(need), _stream()), "ccl_relabel_sequential")
+    ws = torch.empty(max(need.value, 1), dtype=torch.uint8, device=labels.device)
+    count = torch.zeros(1, dtype=torch.int64, device=labels.device)
+    _check(lib.ccl_relabel_sequential(n, _dev(labels, torch.int32, "labels"), _dev(out, torch.int32, "out"),
+                                      count.data_ptr(), ws.data_ptr(), C.byref(need), _stream()), "ccl_relabel_sequential")
+    return out, int(count.item())
 
 
 def _host(t, what):

@@ -92,3 +92,22 @@ def test_wrap_closed_forms():
         zig[3 * (1 * L + x) + 0] = 1
         zig[3 * (1 * L + x) + 1] = 1
     assert oracle.wrap(n, src, dst, dx, dy, zig) == (True, False)
+
+
+def test_relabel_sequential_against_numpy_unique_and_brute_force():
+    """PAPER.md:115.  Pins: np.unique's inverse (sorted distinct labels = clusters in ascending order of smallest site)
+    and a brute-force count on tiny inputs."""
+    rng = np.random.default_rng(115)
+    for trial in range(50):
+        n = int(rng.integers(1, 400))
+        m = int(rng.integers(0, 2 * n))
+        src, dst = graphs.random_graph(rng, n, m, self_loops=True)
+        labels = oracle.label(n, src, dst) if m else np.arange(n, dtype=np.int32)
+        seq, c = oracle.relabel_sequential(labels)
+        uniq, inv = np.unique(labels, return_inverse=True)
+        assert c == uniq.size and np.array_equal(seq, inv)
+        if n <= 60:
+            roots = [i for i in range(n) if labels[i] == i]
+            assert [sum(1 for r in roots if r < labels[i]) for i in range(n)] == seq.tolist()
+    seq, c = oracle.relabel_sequential(np.zeros(0, dtype=np.int32))
+    assert c == 0 and seq.size == 0
