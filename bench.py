@@ -32,6 +32,11 @@ WORKLOADS = {
     "cfg3": ("honeycomb", 4096, 0, [0.60, 0.6527, 0.70], "bits", 3),
     "cfg4": ("regular", 1 << 24, 3, [0.5], "bits", 4),
     "cfg5": ("regular", 1 << 26, 4, [0.25, 1.0 / 3.0, 0.45], "bits", 5),
+    # SURVEY.md 8(f) rows, not BASELINE.json configs: the paper's own Bethe workload (Cayley tree z = 3,
+    # N = 3*2^22 - 2, p = 0.5/1/1.5 p_c, standard and random numbering) and config 1 as a batch of realizations
+    "cayley_std": ("cayley", 22, 0, [0.25, 0.5, 0.75], "bits", 6),
+    "cayley_rand": ("cayley", 22, 1, [0.25, 0.5, 0.75], "bits", 7),
+    "cfg1_batch": ("honeycomb_batch", 64, 4096, [0.6527], "bits", 1),
 }
 METRIC = "Gbonds/s labeled (1 B200) and achieved HBM GB/s fraction of roofline"
 SEED_BASE = 0x1603083570000000          # DESIGN.md input recipe: seed = SEED_BASE + config number
@@ -43,6 +48,13 @@ def describe(name):
     if fam == "regular":
         n, m = size, size * z // 2
         text = "cfg%d random %d-regular N=2^%d M=%d" % (cfg, z, size.bit_length() - 1, m)
+    elif fam == "cayley":
+        n = 3 * (1 << size) - 2
+        m = n - 1
+        text = "Cayley tree z=3 g=%d (%s numbering) N=%d M=%d" % (size, "random" if z else "standard", n, m)
+    elif fam == "honeycomb_batch":
+        n, m = 2 * size * size, 3 * size * size
+        text = "cfg1 honeycomb L=%d periodic N=%d M=%d x %d realizations per call (ccl_label_batch)" % (size, n, m, z)
     else:
         n = (2 if fam == "honeycomb" else 1) * size * size
         m = 3 * size * size
@@ -66,57 +78,54 @@ def measured_peak():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
-    QUERY = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons DURING the timed region (B200_PROFILING.md recipe), sampled through NVML from a
+    thread every ~2 ms (nvidia-smi -lms needs longer to start than a whole timed region lasts here)."""
+    REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
     def __init__(self, index):
         self.index = index
-        self.proc = None
-        self.path = None
+        self.samples, self.reasons, self.smax = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        self._h = None
 
     def start(self):
         try:
-            fd, self.path = tempfile.mkstemp(suffix=".csv")
-            os.close(fd)
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.QUERY,
-                                          "--format=csv,noheader,nounits", "-lms", "20"],
-                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+            import pynvml
+            pynvml.nvmlInit()
+            visible = os.environ.get("CUDA_VISIBLE_DEVICES")
+            idx = int(visible.split(",")[self.index]) if visible and visible.split(",")[self.index].isdigit() else self.index
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.smax = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
         except Exception:
-            self.proc = None
+            self._h = None
+            return
+
+        def run():
+            import pynvml
+            while not self._stop.is_set():
+                try:
+                    self.samples.append(float(pynvml.nvmlDeviceGetClockInfo(self._h, pynvml.NVML_CLOCK_SM)))
+                    r = pynvml.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+                    for name, bit in self.REASONS.items():
+                        if r & bit:
+                            self.reasons.add(name)
+                except Exception:
+                    pass
+                time.sleep(0.002)
+        self._thread = threading.Thread(target=run, daemon=True)
+        self._thread.start()
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.proc is None:
+        out = {"sm_mhz": None, "sm_max_mhz": self.smax, "reasons": [], "samples": 0, "how": "NVML, 2 ms period"}
+        if self._thread is None:
             return out
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except Exception:
-            self.proc.kill()
-        sm, smax, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        try:
-            with open(self.path) as f:
-                for line in f:
-                    parts = [t.strip() for t in line.split(",")]
-                    if len(parts) < 6:
-                        continue
-                    try:
-                        sm.append(float(parts[0]))
-                        smax.append(float(parts[1]))
-                    except ValueError:
-                        continue
-                    for nme, val in zip(names, parts[2:6]):
-                        if val.lower().startswith("active"):
-                            reasons.add(nme)
-            os.unlink(self.path)
-        except Exception:
-            pass
+        self._stop.set()
+        self._thread.join(timeout=2)
+        sm = sorted(self.samples)
         if sm:
-            sm.sort()
-            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(smax), samples=len(sm))
-        out["reasons"] = sorted(reasons)
+            out.update(sm_mhz=sm[len(sm) // 2], samples=len(sm))
+        out["reasons"] = sorted(self.reasons)
         return out
 
 
@@ -131,12 +140,21 @@ def cpu_oracle_sample(name, steps, warmup):
         n = min(size, 1 << CPU_SAMPLE_LOG2_SITES)
         src, dst, _ = oracle.gen_regular(n, z, seed)
         sample = "random %d-regular graph, N=2^%d sites, M=%d bonds" % (z, n.bit_length() - 1, src.size)
+    elif fam == "cayley":
+        g = min(size, 20)
+        n = 3 * (1 << g) - 2
+        perm = np.random.default_rng(seed & 0x7FFFFFFF).permutation(n).astype(np.int32) if z else None
+        n, src, dst = oracle.gen_cayley3(g, perm)
+        sample = "Cayley tree z=3 g=%d (%s numbering), N=%d sites, M=%d bonds" % (g, "random" if z else "standard", n, src.size)
     else:
         L = min(size, 1024)
-        src, dst = (oracle.gen_honeycomb if fam == "honeycomb" else oracle.gen_triangular)(L)
-        n = (2 if fam == "honeycomb" else 1) * L * L
+        src, dst = (oracle.gen_honeycomb if fam.startswith("honeycomb") else oracle.gen_triangular)(L)
+        n = (2 if fam.startswith("honeycomb") else 1) * L * L
         sample = "%s L=%d, N=%d sites, M=%d bonds" % (fam, L, n, src.size)
-    masks = [oracle.gen_occupancy(src.size, p, seed, 0) for p in ps]
+    reps = 256 if fam == "honeycomb_batch" else 1           # a bounded sample of the batch: 256 realizations per p
+    masks = [oracle.gen_occupancy(src.size, p, seed, r) for p in ps for r in range(reps)]
+    if reps > 1:
+        sample += " x %d realizations" % reps
     times = []
     for it in range(warmup + steps):
         t0 = time.perf_counter()
@@ -150,7 +168,7 @@ def cpu_oracle_sample(name, steps, warmup):
     per_step = sum(times) / len(times)
     sample += ", p sweep " + ",".join("%.4g" % p for p in ps) + ", same seeds; labeling time only (oracle_label%s)" % (
         "" if kind == "u8" else "_bits")
-    return len(ps) * src.size / per_step / 1e9, per_step, sample
+    return len(masks) * src.size / per_step / 1e9, per_step, sample
 
 
 def replica_plan(rank, cfg):
@@ -220,24 +238,41 @@ def run_ours(args):
         k, v = kv.split("=")
         ccl.set_option(k, int(v))
     # ---- synthetic inputs, generated on the device by the library's own seeded generators (untimed)
+    batch = z if fam == "honeycomb_batch" else 1            # realizations labeled per call
     if fam == "regular":
         src, dst = ccl.gen_regular(n, z, seed)
-    elif fam == "honeycomb":
+    elif fam == "cayley":
+        perm = None
+        if z:                                               # "random" numbering: a seeded permutation
+            gen = torch.Generator(device="cuda")
+            gen.manual_seed(seed & 0x7FFFFFFF)
+            perm = torch.randperm(n, device="cuda", generator=gen).to(torch.int32)
+        _, src, dst = ccl.gen_cayley3(size, perm)
+    elif fam.startswith("honeycomb"):
         src, dst = ccl.gen_honeycomb(size)
     else:
         src, dst = ccl.gen_triangular(size)
     masks = []
     plan = replica_plan(rank, cfg)
     for p in ps:                      # replicas differ by realization = rank
+        if batch > 1:
+            words = (m + 31) // 32
+            bits = torch.empty((batch, words), dtype=torch.int32, device="cuda")
+            for r in range(batch):
+                bits[r] = ccl.gen_occupancy(m, p, plan["seed"], plan["realization"] * batch + r, want_mask=False)[1]
+            masks.append(bits)
+            continue
         mask, bits = ccl.gen_occupancy(m, p, plan["seed"], plan["realization"], want_mask=(kind == "u8"),
                                        want_bits=(kind != "u8"))
         masks.append(mask if kind == "u8" else bits)
-    labels = torch.empty(n, dtype=torch.int32, device="cuda")
+    labels = torch.empty(n * batch, dtype=torch.int32, device="cuda")
     torch.cuda.synchronize()
     torch.cuda.empty_cache()
 
     def one_call(k):
-        if kind == "u8":
+        if batch > 1:
+            ccl.label_batch(n, src, dst, masks[k], batch, labels=labels.view(batch, n))
+        elif kind == "u8":
             ccl.label(n, src, dst, masks[k], labels=labels)
         else:
             ccl.label_bits(n, src, dst, masks[k], labels=labels)
@@ -275,9 +310,14 @@ def run_ours(args):
             if flush is not None:
                 flush.fill_(c & 0xFF)
             e = ev[c]
-            ccl.set_profile_events(e[1], e[2], e[3])
-            e[0].record()
-            one_call(k)
+            if batch > 1:                             # one kernel does steps (i)-(iv): no per-step events
+                e[0].record(); e[1].record()
+                one_call(k)
+                e[2].record(); e[3].record()
+            else:
+                ccl.set_profile_events(e[1], e[2], e[3])
+                e[0].record()
+                one_call(k)
             c += 1
     t_stop.record()
     barrier()
@@ -293,11 +333,14 @@ def run_ours(args):
         total_ms = sum(call_ms)                       # exclude the flush writes from the step time
     total_ms = max_over_ranks(total_ms, world, "cuda")
     ms_per_step = total_ms / K
-    value = job_value(world, len(ps), m, ms_per_step)
+    value = job_value(world, len(ps), m * batch, ms_per_step)
 
     peak, peak_src = measured_peak()
     avg = lambda xs: sum(xs) / len(xs)
     stream_bytes = 8 * m + (m if kind == "u8" else 4 * ((m + 31) // 32))
+    call_bytes = min_bytes(n, m, kind)
+    if batch > 1:            # per call: the bond list once, a mask and 12 N of label traffic per realization
+        stream_bytes = call_bytes = 8 * m + batch * (4 * ((m + 31) // 32) + 12 * n)
     ach = stream_bytes / (avg(reduce_ms) * 1e-3) / 1e9
     traffic = None
     try:
@@ -305,20 +348,20 @@ def run_ours(args):
             traffic = json.load(f).get(args.workload, {}).get("k_reduce_dram_bytes_per_launch")
     except Exception:
         pass
-    call_ach = min_bytes(n, m, kind) / (avg(call_ms) * 1e-3) / 1e9
+    call_ach = call_bytes / (avg(call_ms) * 1e-3) / 1e9
     per_p = {}
     for k, p in enumerate(ps):
         sel = [i for i in range(ncalls) if i % len(ps) == k]
         t = avg([call_ms[i] for i in sel])
         per_p["%.4g" % p] = {"ms": t, "init_ms": avg([init_ms[i] for i in sel]),
                              "reduce_ms": avg([reduce_ms[i] for i in sel]), "flatten_ms": avg([flat_ms[i] for i in sel]),
-                             "gbonds_per_s": m / (t * 1e-3) / 1e9, "gsites_per_s": n / (t * 1e-3) / 1e9,
-                             "roofline_frac_measured": min_bytes(n, m, kind) / (t * 1e-3) / 1e9 / peak,
-                             "roofline_frac_8TBs": min_bytes(n, m, kind) / (t * 1e-3) / 1e9 / 8000.0}
+                             "gbonds_per_s": m * batch / (t * 1e-3) / 1e9, "gsites_per_s": n * batch / (t * 1e-3) / 1e9,
+                             "roofline_frac_measured": call_bytes / (t * 1e-3) / 1e9 / peak,
+                             "roofline_frac_8TBs": call_bytes / (t * 1e-3) / 1e9 / 8000.0}
 
     # ---- end to end through the host-buffer entry point: H2D of the inputs and D2H of the labels inside the timing
     e2e = None
-    if not args.no_e2e and kind != "u8":
+    if not args.no_e2e and kind != "u8" and batch == 1:
         hs, hd = src.cpu().pin_memory(), dst.cpu().pin_memory()
         hm = [b.cpu().pin_memory() for b in masks]
         hl = torch.empty(n, dtype=torch.int32).pin_memory()
@@ -350,18 +393,18 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": "Gbonds/s", "n_gpus": world, "steps": K,
             "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": text, "calls_per_step": len(ps), "api": "ccl_label" if kind == "u8" else "ccl_label_bits",
+            "config": {"workload": text, "calls_per_step": len(ps), "api": "ccl_label_batch" if batch > 1 else "ccl_label" if kind == "u8" else "ccl_label_bits",
                        "parallelism": "replicas x%d (one realization per GPU, no collective)" % world,
                        "l2": "inputs larger than L2 (bond stream %.0f MB per call vs 126 MB L2)" % (stream_bytes / 1e6)
                        if flush is None else "256 MB buffer rewritten between timed calls (L2 flush)",
-                       "gsites_per_s": world * len(ps) * n / (ms_per_step * 1e-3) / 1e9},
-            "roofline": {"bound": "hbm", "kernel": "k_reduce (step iii)", "achieved": ach, "peak": peak, "unit": "GB/s",
+                       "gsites_per_s": world * len(ps) * n * batch / (ms_per_step * 1e-3) / 1e9},
+            "roofline": {"bound": "hbm", "kernel": "k_label_batch (steps i-iv)" if batch > 1 else "step (iii): k_reduce, or k_scatter + k_descend x regions", "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": stream_bytes, "avg_launch_ms": avg(reduce_ms),
                          "share_of_call": avg(reduce_ms) / avg(call_ms)},
             "roofline_call": {"bound": "hbm", "what": "whole ccl_label call, B_min = 8M + mask + 12N (SURVEY 8(d))",
                               "achieved": call_ach, "peak": peak, "unit": "GB/s", "frac": call_ach / peak,
-                              "frac_of_8TBs_nominal": call_ach / 8000.0, "bytes_per_call": min_bytes(n, m, kind),
+                              "frac_of_8TBs_nominal": call_ach / 8000.0, "bytes_per_call": call_bytes,
                               "avg_call_ms": avg(call_ms)},
             "per_p": per_p, "kernel_ms": {"k_init": avg(init_ms), "k_reduce": avg(reduce_ms), "k_flatten": avg(flat_ms)},
             "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,

@@ -81,6 +81,13 @@ int ccl_validate_bonds(int64_t n_sites, int64_t n_bonds, const int32_t* src, con
 int ccl_gen_triangular(int32_t L, int32_t* src, int32_t* dst, void* stream);
 int ccl_gen_honeycomb(int32_t L, int32_t* src, int32_t* dst, void* stream);
 
+/* Cayley tree with coordination number 3 and g generations -- the paper's own "Bethe lattice" workload
+ * (PAPER.md:189-193): N = 3*2^g - 2 sites, N - 1 bonds; site 0 has children 1, 2, 3 and site i >= 1 has children
+ * 2i+2, 2i+3 ("standard position" numbering, R11); bond k joins site k+1 (dst) to its parent (src).
+ * perm_or_null: device int32[N] permutation giving the "random" numbering (site i is called perm[i]); NULL = standard.
+ * 1 <= g <= 28. */
+int ccl_gen_cayley3(int32_t g, const int32_t* perm_or_null, int32_t* src, int32_t* dst, void* stream);
+
 /* Simple random z-regular graph on n_sites sites by the configuration model ("Bethe substitute" of
  * BASELINE.json configs 4-5; the paper's own Bethe workload is the Cayley tree):
  * n_sites*z/2 bonds in uniformly random order; stub keys from Philox4x32-10, stable sort, defects (self-loops,

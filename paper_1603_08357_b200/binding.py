@@ -14,7 +14,8 @@ lib = C.CDLL(_LIB_PATH)
 
 EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangular", "ccl_gen_honeycomb",
            "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
-           "ccl_set_profile_events", "ccl_set_option", "ccl_label_batch", "ccl_relabel_sequential", "ccl_last_error",
+           "ccl_set_profile_events", "ccl_set_option", "ccl_label_batch", "ccl_relabel_sequential", "ccl_gen_cayley3",
+           "ccl_last_error",
            "ccl_version", "ccl_launch_count"]
 
 _vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
@@ -36,7 +37,8 @@ lib.ccl_set_profile_events.argtypes = [_vp, _vp, _vp]
 lib.ccl_set_option.argtypes = [C.c_char_p, _i64]
 lib.ccl_label_batch.argtypes = [_i64, _i64, _vp, _vp, _vp, _i64, _i32, _vp, _vp]
 lib.ccl_relabel_sequential.argtypes = [_i64, _vp, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
-for _n in EXPORTS[:13]:
+lib.ccl_gen_cayley3.argtypes = [_i32, _vp, _vp, _vp, _vp]
+for _n in EXPORTS[:14]:
     getattr(lib, _n).restype = C.c_int
 
 
@@ -184,6 +186,16 @@ def gen_triangular(L, device="cuda"):
 
 def gen_honeycomb(L, device="cuda"):
     return _lattice(lib.ccl_gen_honeycomb, "ccl_gen_honeycomb", L, device)
+
+
+def gen_cayley3(g, perm=None, device="cuda"):
+    """ccl_gen_cayley3: (n_sites, src, dst) of the z = 3 Cayley tree with g generations; perm = int32 CUDA permutation."""
+    n = 3 * (1 << g) - 2
+    src = torch.empty(n - 1, dtype=torch.int32, device=device)
+    dst = torch.empty(n - 1, dtype=torch.int32, device=device)
+    _check(lib.ccl_gen_cayley3(g, _dev(perm, torch.int32, "perm"), src.data_ptr(), dst.data_ptr(), _stream()),
+           "ccl_gen_cayley3")
+    return n, src, dst
 
 
 def gen_regular(n_sites, z, seed, device="cuda"):

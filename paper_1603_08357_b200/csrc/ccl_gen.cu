@@ -222,6 +222,32 @@ extern "C" int ccl_gen_honeycomb(int32_t L, int32_t* src, int32_t* dst, void* st
     return CCL_OK;
 }
 
+// Cayley tree with coordination number 3 (the paper's "Bethe lattice", R11): site 0 has
+// children 1, 2, 3; site i >= 1 has children 2i+2, 2i+3.  Bond k joins site k+1 to its parent.
+namespace ccl {
+__global__ void __launch_bounds__(kGenThreads)
+k_gen_cayley3(int64_t n_bonds, const int32_t* __restrict__ perm, int32_t* __restrict__ src, int32_t* __restrict__ dst)
+{
+    const int64_t stride = (int64_t)gridDim.x * kGenThreads;
+    for (int64_t k = (int64_t)blockIdx.x * kGenThreads + threadIdx.x; k < n_bonds; k += stride) {
+        const int64_t child = k + 1, parent = child <= 3 ? 0 : (child - 2) / 2;
+        src[k] = perm ? perm[parent] : (int32_t)parent;
+        dst[k] = perm ? perm[child] : (int32_t)child;
+    }
+}
+}  // namespace ccl
+
+extern "C" int ccl_gen_cayley3(int32_t g, const int32_t* perm_or_null, int32_t* src, int32_t* dst, void* stream)
+{
+    using namespace ccl;
+    CCL_REQUIRE(g >= 1 && g <= 28, "g out of range [1, 28]");
+    CCL_REQUIRE(src && dst, "src/dst is NULL");
+    const int64_t n_bonds = 3 * ((int64_t)1 << g) - 3;
+    k_gen_cayley3<<<(unsigned)grid_for(n_bonds), kGenThreads, 0, as_stream(stream)>>>(n_bonds, perm_or_null, src, dst);
+    CCL_CHECK_LAUNCH("k_gen_cayley3");
+    return CCL_OK;
+}
+
 extern "C" int ccl_gen_occupancy(int64_t n_bonds, double p, uint64_t seed, uint32_t realization,
                                  uint8_t* mask_or_null, uint32_t* bits_or_null, void* stream)
 {

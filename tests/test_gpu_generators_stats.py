@@ -101,3 +101,21 @@ def test_pipeline_on_device_matches_oracle_pipeline(ccl):
     wl = oracle.label(L * L, ws, wd, wm)
     assert np.array_equal(lab.cpu().numpy(), wl)
     assert ccl.cluster_stats(lab)[0] == oracle.stats(wl)[0]
+
+
+@pytest.mark.parametrize("g", [1, 2, 5, 16])
+def test_cayley_generator(ccl, g):
+    """PAPER.md:189-193 workload: device generator == oracle generator, standard and random numbering."""
+    n, src, dst = ccl.gen_cayley3(g)
+    wn, wsrc, wdst = oracle.gen_cayley3(g)
+    assert n == wn == 3 * (1 << g) - 2
+    assert np.array_equal(src.cpu().numpy(), wsrc) and np.array_equal(dst.cpu().numpy(), wdst)
+    perm = np.random.default_rng(g).permutation(n).astype(np.int32)
+    _, src, dst = ccl.gen_cayley3(g, torch.from_numpy(perm).cuda())
+    _, wsrc, wdst = oracle.gen_cayley3(g, perm)
+    assert np.array_equal(src.cpu().numpy(), wsrc) and np.array_equal(dst.cpu().numpy(), wdst)
+    # a forest at every p: clusters = N - occupied bonds (SURVEY 8(c))
+    mask, bits = oracle.gen_occupancy(n - 1, 0.5, oracle.seed_for(6))
+    lab = ccl.label(n, src, dst, torch.from_numpy(mask).cuda())
+    stats, _, _ = ccl.cluster_stats(lab, 0)
+    assert stats["n_clusters"] == n - int(mask.sum())
