@@ -120,6 +120,24 @@ int ccl_cluster_stats(int64_t n_sites, const int32_t* labels, int32_t* size_scra
 int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_src, const int32_t* host_dst,
                         const uint32_t* host_occupied_bits, int32_t* host_labels, void* stream);
 
+/* ---- wrapping on a periodic lattice (reading R7 of "spanning") ---------------
+ *
+ * ccl_gen_wrap_vectors: per bond of ccl_gen_triangular (family 0) / ccl_gen_honeycomb (family 1), in the same bond
+ * order, how many times the bond crosses the periodic seam from src to dst along x and along y (0 or 1 here; ccl_wrap
+ * accepts -1, 0, 1).  int8 [3*L*L] each.
+ *
+ * ccl_wrap: out[0] = 1 iff some cluster of the occupied graph holds a closed path with non-zero winding along x, out[1]
+ * the same along y, out[2] = 1 iff an internal 16-bit sheet offset overflowed (result invalid; needs > 32000 seam
+ * crossings on one path), out[3] = 0.  out: device int32[4].  Method: labels_open (device int32[n_sites], output)
+ * receives the canonical labels of the OPEN lattice (occupied bonds with a zero wrap vector, through ccl_label_bits);
+ * the occupied seam bonds then run a lock-free weighted union-find over the open clusters.  wx, wy: device int8
+ * [n_bonds], 16-byte aligned.  occupied_bits as in ccl_label_bits (NULL = all occupied).  workspace: call with
+ * workspace == NULL for the size in *workspace_bytes (host pointer); 256-byte aligned device memory. */
+int ccl_gen_wrap_vectors(int32_t family, int32_t L, int8_t* wx, int8_t* wy, void* stream);
+int ccl_wrap(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const uint32_t* occupied_bits,
+             const int8_t* wx, const int8_t* wy, int32_t* labels_open, int32_t* out, void* workspace,
+             size_t* workspace_bytes, void* stream);
+
 /* ---- many realizations of one small graph in one launch ---------------------------
  *
  * The same bond list (src, dst, n_bonds) under n_batch packed occupancy masks: realization r reads the mask at

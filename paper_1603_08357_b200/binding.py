@@ -15,7 +15,7 @@ lib = C.CDLL(_LIB_PATH)
 EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangular", "ccl_gen_honeycomb",
            "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
            "ccl_set_profile_events", "ccl_set_option", "ccl_label_batch", "ccl_relabel_sequential", "ccl_gen_cayley3",
-           "ccl_last_error",
+           "ccl_gen_wrap_vectors", "ccl_wrap", "ccl_last_error",
            "ccl_version", "ccl_launch_count"]
 
 _vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
@@ -38,7 +38,9 @@ lib.ccl_set_option.argtypes = [C.c_char_p, _i64]
 lib.ccl_label_batch.argtypes = [_i64, _i64, _vp, _vp, _vp, _i64, _i32, _vp, _vp]
 lib.ccl_relabel_sequential.argtypes = [_i64, _vp, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
 lib.ccl_gen_cayley3.argtypes = [_i32, _vp, _vp, _vp, _vp]
-for _n in EXPORTS[:14]:
+lib.ccl_gen_wrap_vectors.argtypes = [_i32, _i32, _vp, _vp, _vp]
+lib.ccl_wrap.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
+for _n in EXPORTS[:16]:
     getattr(lib, _n).restype = C.c_int
 
 
@@ -186,6 +188,33 @@ def gen_triangular(L, device="cuda"):
 
 def gen_honeycomb(L, device="cuda"):
     return _lattice(lib.ccl_gen_honeycomb, "ccl_gen_honeycomb", L, device)
+
+
+def gen_wrap_vectors(family, L, device="cuda"):
+    """ccl_gen_wrap_vectors: (wx, wy) int8 tensors for the bonds of gen_triangular ("triangular") / gen_honeycomb."""
+    fam = {"triangular": 0, "honeycomb": 1}[family]
+    wx = torch.empty(3 * L * L, dtype=torch.int8, device=device)
+    wy = torch.empty(3 * L * L, dtype=torch.int8, device=device)
+    _check(lib.ccl_gen_wrap_vectors(fam, L, wx.data_ptr(), wy.data_ptr(), _stream()), "ccl_gen_wrap_vectors")
+    return wx, wy
+
+
+def wrap(n_sites, src, dst, occupied_bits, wx, wy, labels_open=None):
+    """ccl_wrap: (wrap_x, wrap_y, labels_open).  Reads the flags back (synchronises)."""
+    if labels_open is None:
+        labels_open = torch.empty(n_sites, dtype=torch.int32, device=src.device)
+    need = C.c_size_t(0)
+    _check(lib.ccl_wrap(n_sites, src.numel(), None, None, None, None, None, None, None, None, C.byref(need), _stream()), "ccl_wrap")
+    ws = torch.empty(need.value, dtype=torch.uint8, device=src.device)
+    out = torch.zeros(4, dtype=torch.int32, device=src.device)
+    _check(lib.ccl_wrap(n_sites, src.numel(), _dev(src, torch.int32, "src"), _dev(dst, torch.int32, "dst"),
+                        _dev(occupied_bits, torch.int32, "occupied_bits"), _dev(wx, torch.int8, "wx"), _dev(wy, torch.int8, "wy"),
+                        _dev(labels_open, torch.int32, "labels_open"), out.data_ptr(), ws.data_ptr(), C.byref(need), _stream()),
+           "ccl_wrap")
+    flags = out.cpu().tolist()
+    if flags[2]:
+        raise CclError(3, "ccl_wrap (sheet offset overflow)")
+    return bool(flags[0]), bool(flags[1]), labels_open
 
 
 def gen_cayley3(g, perm=None, device="cuda"):

@@ -222,6 +222,38 @@ extern "C" int ccl_gen_honeycomb(int32_t L, int32_t* src, int32_t* dst, void* st
     return CCL_OK;
 }
 
+// Wrap vectors of the lattice bonds (how often bond b crosses the periodic seam from src to dst, per axis), in the bond
+// order of k_gen_triangular / k_gen_honeycomb.  Input of ccl_wrap.
+namespace ccl {
+__global__ void __launch_bounds__(kGenThreads)
+k_gen_wrap_vectors(int family, int32_t L, int8_t* __restrict__ wx, int8_t* __restrict__ wy)
+{
+    const int64_t n_bonds = 3ll * L * L;
+    const int64_t stride = (int64_t)gridDim.x * kGenThreads;
+    for (int64_t b = (int64_t)blockIdx.x * kGenThreads + threadIdx.x; b < n_bonds; b += stride) {
+        const int64_t cell = b / 3;
+        const int k = (int)(b - 3 * cell);
+        const int32_t x = (int32_t)(cell % L), y = (int32_t)(cell / L);
+        int sx, sy;                                    // the bond's step in cells
+        if (family == 0) { sx = (k != 1); sy = (k != 0); }          // triangular: (1,0), (0,1), (1,1)
+        else { sx = (k == 1); sy = (k == 2); }                      // honeycomb: A-B in the cell, B-A(x+1,y), B-A(x,y+1)
+        wx[b] = (int8_t)(x + sx >= L);
+        wy[b] = (int8_t)(y + sy >= L);
+    }
+}
+}  // namespace ccl
+
+extern "C" int ccl_gen_wrap_vectors(int32_t family, int32_t L, int8_t* wx, int8_t* wy, void* stream)
+{
+    using namespace ccl;
+    CCL_REQUIRE(family == 0 || family == 1, "family must be 0 (triangular) or 1 (honeycomb)");
+    CCL_REQUIRE(L >= 1 && 2ll * L * L <= 2147483647LL, "L out of range");
+    CCL_REQUIRE(wx && wy, "wx/wy is NULL");
+    k_gen_wrap_vectors<<<(unsigned)grid_for(3ll * L * L), kGenThreads, 0, as_stream(stream)>>>(family, L, wx, wy);
+    CCL_CHECK_LAUNCH("k_gen_wrap_vectors");
+    return CCL_OK;
+}
+
 // Cayley tree with coordination number 3 (the paper's "Bethe lattice", R11): site 0 has
 // children 1, 2, 3; site i >= 1 has children 2i+2, 2i+3.  Bond k joins site k+1 to its parent.
 namespace ccl {

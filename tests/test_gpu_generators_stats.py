@@ -119,3 +119,57 @@ def test_cayley_generator(ccl, g):
     lab = ccl.label(n, src, dst, torch.from_numpy(mask).cuda())
     stats, _, _ = ccl.cluster_stats(lab, 0)
     assert stats["n_clusters"] == n - int(mask.sum())
+
+
+def _wrap_vectors_from_oracle(family, L):
+    """Wrap vectors derived on the test side from the oracle generator's displacements: the bond leaves cell (x, y) by
+    (dx, dy) cells; it crosses the seam iff the target cell lies outside [0, L)."""
+    src, dst, dx, dy = (oracle.gen_triangular if family == "triangular" else oracle.gen_honeycomb)(L, with_disp=True)
+    cell = src.astype(np.int64) // (2 if family == "honeycomb" else 1)
+    wx = ((cell % L + dx) // L).astype(np.int8)
+    wy = ((cell // L + dy) // L).astype(np.int8)
+    return src, dst, dx, dy, wx, wy
+
+
+@pytest.mark.parametrize("family", ["triangular", "honeycomb"])
+def test_wrapping_detection_small_lattices(ccl, family):
+    """GPU: open-lattice labels + lock-free weighted union-find over the seam bonds.  Oracle: displacement union-find
+    over all bonds (pinned by BFS on the unwrapped cover).  Different formulations, same answer, 1200 realizations."""
+    pc = 0.3473 if family == "triangular" else 0.6527
+    seen = set()
+    for L in (1, 2, 3, 4, 5, 7, 9, 16, 33):
+        src, dst, dx, dy, wx, wy = _wrap_vectors_from_oracle(family, L)
+        gx, gy = ccl.gen_wrap_vectors(family, L)
+        assert np.array_equal(gx.cpu().numpy(), wx) and np.array_equal(gy.cpu().numpy(), wy)
+        n = (2 if family == "honeycomb" else 1) * L * L
+        s, d = torch.from_numpy(src).cuda(), torch.from_numpy(dst).cuda()
+        for r in range(70):
+            p = [0.0, 1.0, pc, pc - 0.1, pc + 0.1, pc + 0.03, pc - 0.03][r % 7]
+            mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(3), realization=r)
+            want = oracle.wrap(n, src, dst, dx, dy, mask)
+            got_x, got_y, lab_open = ccl.wrap(n, s, d, torch.from_numpy(bits.view(np.int32)).cuda(), gx, gy)
+            assert (got_x, got_y) == want, (L, p, r)
+            open_mask = mask & ((wx == 0) & (wy == 0)).astype(np.uint8)
+            assert np.array_equal(lab_open.cpu().numpy(), oracle.label(n, src, dst, open_mask))
+            seen.add(want)
+    assert len(seen) == 4                                   # none, x only, y only, both all occurred
+
+
+@pytest.mark.parametrize("family,L", [("triangular", 257), ("honeycomb", 301)])
+def test_wrapping_detection_larger_lattices(ccl, family, L):
+    pc = 0.3473 if family == "triangular" else 0.6527
+    src, dst, dx, dy, wx, wy = _wrap_vectors_from_oracle(family, L)
+    n = (2 if family == "honeycomb" else 1) * L * L
+    s, d = torch.from_numpy(src).cuda(), torch.from_numpy(dst).cuda()
+    gx, gy = torch.from_numpy(wx).cuda(), torch.from_numpy(wy).cuda()
+    for r, p in enumerate([pc - 0.02, pc - 0.005, pc, pc, pc, pc + 0.005, pc + 0.02, 1.0]):
+        mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(3), realization=r)
+        got = ccl.wrap(n, s, d, torch.from_numpy(bits.view(np.int32)).cuda(), gx, gy)[:2]
+        assert got == oracle.wrap(n, src, dst, dx, dy, mask), (p, r)
+    # all bonds occupied without a mask; a single occupied row wraps in x only
+    assert ccl.wrap(n, s, d, None, gx, gy)[:2] == (True, True)
+    if family == "triangular":
+        row = np.zeros(src.size, dtype=np.uint8)
+        row[3 * np.arange(5 * L, 6 * L)] = 1                # bonds k = 0 of row y = 5
+        got = ccl.wrap(n, s, d, torch.from_numpy(graphs.pack_bits(row).view(np.int32)).cuda(), gx, gy)[:2]
+        assert got == (True, False) == oracle.wrap(n, src, dst, dx, dy, row)
