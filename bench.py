@@ -382,6 +382,25 @@ def run_ours(args):
                "api": "ccl_label_bits_host (pinned host src/dst/bits in, host labels out, synchronous)"}
         del hs, hd, hm, hl
 
+    # ---- config 3 asks for "largest-cluster and wrapping statistics per p": untimed, after the timed region
+    statistics = None
+    if rank == 0 and fam in ("triangular", "honeycomb") and kind != "u8":
+        statistics = {}
+        wx, wy = ccl.gen_wrap_vectors(fam, size)
+        for k, p in enumerate(ps):
+            t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True); t2 = torch.cuda.Event(enable_timing=True)
+            one_call(k)
+            t0.record()
+            st, _, _ = ccl.cluster_stats(labels, 0)
+            t1.record()
+            wrap_x, wrap_y, _ = ccl.wrap(n, src, dst, masks[k], wx, wy)
+            t2.record()
+            torch.cuda.synchronize()
+            statistics["%.4g" % p] = {"n_clusters": st["n_clusters"], "largest": st["largest"], "largest_over_n": st["largest"] / n,
+                                      "wrap_x": wrap_x, "wrap_y": wrap_y, "cluster_stats_ms": t0.elapsed_time(t1),
+                                      "wrap_ms_incl_open_labeling": t1.elapsed_time(t2)}
+        del wx, wy
+
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
         v, per_step, sample = cpu_oracle_sample(args.workload, 3, 1)
@@ -407,7 +426,7 @@ def run_ours(args):
                               "frac_of_8TBs_nominal": call_ach / 8000.0, "bytes_per_call": call_bytes,
                               "avg_call_ms": avg(call_ms)},
             "per_p": per_p, "kernel_ms": {"k_init": avg(init_ms), "k_reduce": avg(reduce_ms), "k_flatten": avg(flat_ms)},
-            "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
+            "statistics": statistics, "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

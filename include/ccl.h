@@ -171,6 +171,9 @@ int ccl_relabel_sequential(int64_t n_sites, const int32_t* labels, int32_t* seq_
  *   "force_mode"              -1 = the probe decides (default), 0 = always direct, 1 = always bucketed when eligible
  *   "bucket_capacity"         pairs each region's bucket can hold (<= 0: 4 M / regions + 4096); pairs that do not
  *                             fit are joined on the spot by the general algorithm
+ *   "two_pass"                direct form of step (iii): 0 = one pass over the bonds, 1 = the paper's order of work
+ *                             (hook every site to its smallest lower neighbour, flatten, then Algorithm 1; two passes
+ *                             over the bonds), -1 = two passes iff n_bonds >= 2.5 n_sites and n_bonds >= 2^20 (default)
  *   "tile_mode"               tiled form of step (iii) for bond lists that are local in the site numbering (window of
  *                             labels in shared memory): 0 = off (default), -1 = a device-side probe
  *                             decides, 1 = always; "sub_shift" (window = 2^value sites, <= 15), "fine_capacity",

@@ -81,6 +81,7 @@ extern "C" int ccl_set_option(const char* name, int64_t value)
         return CCL_OK;
     }
     if (!strcmp(name, "bucket_capacity")) { t.bucket_capacity = value > 0 ? value : 0; return CCL_OK; }
+    if (!strcmp(name, "two_pass")) { t.two_pass = value > 0 ? 1 : value < 0 ? -1 : 0; return CCL_OK; }
     if (!strcmp(name, "tile_mode")) {
         if (value < -1 || value > 1) {
             ccl::set_error("invalid argument: tile_mode must be -1, 0 or 1");

@@ -74,6 +74,8 @@ struct Tuning {                                    // ccl_set_option(); process-
     int32_t region_shift = 23;                     // 2^23 sites = 32 MiB of labels per region
     int32_t force_mode = -1;                       // -1: device-side probe decides; 0: direct; 1: bucketed
     int64_t bucket_capacity = 0;                   // pairs per region bucket; 0 = 4 M / regions + 4096
+    int32_t two_pass = -1;                         // direct form of step (iii): 0 one pass (k_reduce), 1 hook + flatten +
+                                                   // join (the paper's order), -1 by bonds per site (>= 2.5: two passes)
     int32_t tile_mode = 0;                         // tiled form (ccl_tile.cu): 0 off (default: measured slower, see
                                                    // profiles/r1_notes.md), -1 a device-side probe decides, 1 always
     int32_t sub_shift = -1;                        // 2^sub_shift sites per sub-region; -1 = from n_sites

@@ -364,6 +364,30 @@ def test_tiled_form_adversarial(tiled):
         assert np.array_equal(got, oracle.label(n, src, dst, mask))
 
 
+# ------------------------------------------------------------------ two-pass direct form (hook, flatten, join)
+@pytest.mark.parametrize("two_pass", [0, 1])
+def test_two_pass_form(tiled, two_pass):
+    ccl = tiled
+    ccl.set_option("reset")
+    ccl.set_option("two_pass", two_pass)
+    rng = np.random.default_rng(31 + two_pass)
+    for trial in range(40):
+        n = int(rng.integers(2, 50000))
+        m = int(rng.integers(1, 4 * n + 1))
+        src, dst = graphs.random_graph(rng, n, m, self_loops=True)
+        mask = (rng.random(m) < rng.random()).astype(np.uint8)
+        run_all_forms(ccl, n, src, dst, mask)
+    for name in ["honeycomb_L301", "triangular_L257", "regular4", "cayley_random"]:
+        n, src, dst, ps, cfg = _case(name)
+        for p in ps + [1.0]:
+            mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(cfg), realization=9)
+            run_all_forms(ccl, n, src, dst, mask)
+    n = 1 << 18
+    for order in ("ascending", "descending", "shuffled"):
+        src, dst = graphs.path_graph(n, order, rng)
+        assert int(ccl.label(n, dev(src), dev(dst)).max().item()) == 0
+
+
 def test_tuning_argument_checks(ccl):
     with pytest.raises(ccl.CclError):
         ccl.set_tuning(0, 2, 0)
