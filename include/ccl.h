@@ -65,6 +65,14 @@ int ccl_label(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_
 int ccl_label_bits(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
                    const uint32_t* occupied_bits, int32_t* labels, void* stream);
 
+/* The paper's own interface: a nearest-neighbour list instead of a bond list.  nn_list is a dense
+ * z_max x n_sites int32 array, structure of arrays: the k-th neighbour of site i is nn_list[k * n_sites + i]; negative
+ * entries are padding.  Every entry is a connection of the network to be labeled (list it from one side or from both).
+ * The four steps run in the paper's form: (i) label[i] = smallest lower-numbered neighbour, else i; (ii) analysis;
+ * (iii) Algorithm 1 over every (site, lower-numbered neighbour); (iv) analysis.  Same result as ccl_label on the
+ * corresponding bond list.  0 <= z_max <= 1024; neighbours >= n_sites are a caller error (not checked). */
+int ccl_label_nn(int64_t n_sites, int32_t z_max, const int32_t* nn_list, int32_t* labels, void* stream);
+
 /* Debug validator: *out_bad (device int64) = number of bonds with an endpoint outside [0, n_sites). */
 int ccl_validate_bonds(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
                        int64_t* out_bad, void* stream);

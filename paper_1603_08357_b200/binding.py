@@ -15,7 +15,7 @@ lib = C.CDLL(_LIB_PATH)
 EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangular", "ccl_gen_honeycomb",
            "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
            "ccl_set_profile_events", "ccl_set_option", "ccl_label_batch", "ccl_relabel_sequential", "ccl_gen_cayley3",
-           "ccl_gen_wrap_vectors", "ccl_wrap", "ccl_last_error",
+           "ccl_gen_wrap_vectors", "ccl_wrap", "ccl_label_nn", "ccl_last_error",
            "ccl_version", "ccl_launch_count"]
 
 _vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
@@ -40,7 +40,8 @@ lib.ccl_relabel_sequential.argtypes = [_i64, _vp, _vp, _vp, _vp, C.POINTER(C.c_s
 lib.ccl_gen_cayley3.argtypes = [_i32, _vp, _vp, _vp, _vp]
 lib.ccl_gen_wrap_vectors.argtypes = [_i32, _i32, _vp, _vp, _vp]
 lib.ccl_wrap.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
-for _n in EXPORTS[:16]:
+lib.ccl_label_nn.argtypes = [_i64, _i32, _vp, _vp, _vp]
+for _n in EXPORTS[:17]:
     getattr(lib, _n).restype = C.c_int
 
 
@@ -97,6 +98,16 @@ def label_bits(n_sites, src, dst, occupied_bits, labels=None, n_bonds=None):
     _check(lib.ccl_label_bits(n_sites, m, _dev(src, torch.int32, "src"), _dev(dst, torch.int32, "dst"),
                               _dev(occupied_bits, torch.int32, "occupied_bits"),
                               _dev(labels, torch.int32, "labels"), _stream()), "ccl_label_bits")
+    return labels
+
+
+def label_nn(nn_list, labels=None):
+    """ccl_label_nn: nn_list is an int32 CUDA tensor [z_max, n_sites] (negative = padding)."""
+    z_max, n_sites = nn_list.shape
+    if labels is None:
+        labels = torch.empty(n_sites, dtype=torch.int32, device=nn_list.device)
+    _check(lib.ccl_label_nn(n_sites, z_max, _dev(nn_list, torch.int32, "nn_list"), _dev(labels, torch.int32, "labels"),
+                            _stream()), "ccl_label_nn")
     return labels
 
 

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libccl.so")
-SOURCES = ["ccl_api.cu", "ccl_label.cu", "ccl_bucket.cu", "ccl_tile.cu", "ccl_batch.cu", "ccl_wrap.cu", "ccl_gen.cu", "ccl_stats.cu"]
+SOURCES = ["ccl_api.cu", "ccl_label.cu", "ccl_bucket.cu", "ccl_tile.cu", "ccl_batch.cu", "ccl_wrap.cu", "ccl_nn.cu", "ccl_gen.cu", "ccl_stats.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

@@ -320,6 +320,15 @@ static int launch_two_pass(int64_t n_sites, int64_t n_bonds, const int32_t* src,
     return CCL_OK;
 }
 
+// step (ii)/(iv) for the other translation units (ccl_nn.cu)
+int flatten_labels(int64_t n_sites, int32_t* labels, cudaStream_t st)
+{
+    const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
+    k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels);
+    CCL_CHECK_LAUNCH("k_flatten");
+    return CCL_OK;
+}
+
 // Optional per-step CUDA events (ccl_set_profile_events): recorded on the call's stream between the kernels so
 // that a benchmark can read each step's device time from inside its own timed region.
 static thread_local cudaEvent_t g_ev[3] = {nullptr, nullptr, nullptr};

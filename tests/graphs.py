@@ -154,3 +154,24 @@ def same_partition(a, b):
         if fwd.setdefault(x, y) != y or bwd.setdefault(y, x) != x:
             return False
     return True
+
+
+def nn_list_from_bonds(n_sites, src, dst, occupied=None, both_sides=True):
+    """Dense z_max x n_sites nearest-neighbour list (structure of arrays, -1 padding) of the occupied bonds.
+    both_sides: each bond is listed at both of its ends (the paper's form) or only at its higher-numbered end."""
+    keep = np.ones(len(src), dtype=bool) if occupied is None else np.asarray(occupied) != 0
+    u = np.asarray(src)[keep].astype(np.int64)
+    v = np.asarray(dst)[keep].astype(np.int64)
+    if both_sides:
+        a, b = np.concatenate([u, v]), np.concatenate([v, u])
+    else:
+        a, b = np.maximum(u, v), np.minimum(u, v)
+    order = np.argsort(a, kind="stable")
+    a, b = a[order], b[order]
+    deg = np.bincount(a, minlength=n_sites) if a.size else np.zeros(n_sites, dtype=np.int64)
+    z_max = int(deg.max()) if n_sites and a.size else 0
+    nn = np.full((z_max, n_sites), -1, dtype=np.int32)
+    start = np.concatenate([[0], np.cumsum(deg)[:-1]]) if n_sites else np.zeros(0, dtype=np.int64)
+    slot = np.arange(a.size) - start[a] if a.size else np.zeros(0, dtype=np.int64)
+    nn[slot, a] = b
+    return nn
