@@ -37,6 +37,8 @@ WORKLOADS = {
     "cayley_std": ("cayley", 22, 0, [0.25, 0.5, 0.75], "bits", 6),
     "cayley_rand": ("cayley", 22, 1, [0.25, 0.5, 0.75], "bits", 7),
     "cfg1_batch": ("honeycomb_batch", 64, 4096, [0.6527], "bits", 1),
+    # config 2 through the paper's own interface (dense NN list z_max x N, ccl_label_nn), for comparison with the bond list
+    "cfg2_nn": ("triangular_nn", 4096, 0, [0.3473], "bits", 2),
 }
 METRIC = "Gbonds/s labeled (1 B200) and achieved HBM GB/s fraction of roofline"
 SEED_BASE = 0x1603083570000000          # DESIGN.md input recipe: seed = SEED_BASE + config number
@@ -55,6 +57,9 @@ def describe(name):
     elif fam == "honeycomb_batch":
         n, m = 2 * size * size, 3 * size * size
         text = "cfg1 honeycomb L=%d periodic N=%d M=%d x %d realizations per call (ccl_label_batch)" % (size, n, m, z)
+    elif fam == "triangular_nn":
+        n, m = size * size, 3 * size * size
+        text = "cfg2 triangular L=%d periodic N=%d M=%d as a dense NN list (z_max x N int32, ccl_label_nn)" % (size, n, m)
     else:
         n = (2 if fam == "honeycomb" else 1) * size * size
         m = 3 * size * size
@@ -150,7 +155,7 @@ def cpu_oracle_sample(name, steps, warmup):
         L = min(size, 1024)
         src, dst = (oracle.gen_honeycomb if fam.startswith("honeycomb") else oracle.gen_triangular)(L)
         n = (2 if fam.startswith("honeycomb") else 1) * L * L
-        sample = "%s L=%d, N=%d sites, M=%d bonds" % (fam, L, n, src.size)
+        sample = "%s L=%d, N=%d sites, M=%d bonds (bond-list oracle)" % (fam, L, n, src.size)
     reps = 256 if fam == "honeycomb_batch" else 1           # a bounded sample of the batch: 256 realizations per p
     masks = [oracle.gen_occupancy(src.size, p, seed, r) for p in ps for r in range(reps)]
     if reps > 1:
@@ -265,12 +270,30 @@ def run_ours(args):
         mask, bits = ccl.gen_occupancy(m, p, plan["seed"], plan["realization"], want_mask=(kind == "u8"),
                                        want_bits=(kind != "u8"))
         masks.append(mask if kind == "u8" else bits)
+    nn_lists = []
+    if fam == "triangular_nn":          # NN list of the occupied bonds, every bond at both ends, built with torch ops (untimed)
+        for bits in masks:
+            b = torch.arange(m, device="cuda")
+            on = ((bits[b >> 5] >> (b & 31)) & 1).bool()
+            u, v = src[on].long(), dst[on].long()
+            a, c = torch.cat([u, v]), torch.cat([v, u])
+            a, order = torch.sort(a, stable=True)
+            c = c[order]
+            deg = torch.bincount(a, minlength=n)
+            start = torch.cumsum(deg, 0) - deg
+            slot = torch.arange(a.numel(), device="cuda") - start[a]
+            nn = torch.full((int(deg.max().item()), n), -1, dtype=torch.int32, device="cuda")
+            nn[slot, a] = c.to(torch.int32)
+            nn_lists.append(nn)
+            del b, on, u, v, a, c, order, deg, start, slot
     labels = torch.empty(n * batch, dtype=torch.int32, device="cuda")
     torch.cuda.synchronize()
     torch.cuda.empty_cache()
 
     def one_call(k):
-        if batch > 1:
+        if nn_lists:
+            ccl.label_nn(nn_lists[k], labels=labels)
+        elif batch > 1:
             ccl.label_batch(n, src, dst, masks[k], batch, labels=labels.view(batch, n))
         elif kind == "u8":
             ccl.label(n, src, dst, masks[k], labels=labels)
@@ -310,7 +333,7 @@ def run_ours(args):
             if flush is not None:
                 flush.fill_(c & 0xFF)
             e = ev[c]
-            if batch > 1:                             # one kernel does steps (i)-(iv): no per-step events
+            if batch > 1 or nn_lists:                 # no per-step events on these entry points
                 e[0].record(); e[1].record()
                 one_call(k)
                 e[2].record(); e[3].record()
@@ -341,6 +364,8 @@ def run_ours(args):
     call_bytes = min_bytes(n, m, kind)
     if batch > 1:            # per call: the bond list once, a mask and 12 N of label traffic per realization
         stream_bytes = call_bytes = 8 * m + batch * (4 * ((m + 31) // 32) + 12 * n)
+    if nn_lists:             # the NN list is read twice (steps (i) and (iii)) + 12 N of label traffic
+        stream_bytes = call_bytes = 2 * 4 * nn_lists[0].numel() + 12 * n
     ach = stream_bytes / (avg(reduce_ms) * 1e-3) / 1e9
     traffic = None
     try:
@@ -361,7 +386,7 @@ def run_ours(args):
 
     # ---- end to end through the host-buffer entry point: H2D of the inputs and D2H of the labels inside the timing
     e2e = None
-    if not args.no_e2e and kind != "u8" and batch == 1:
+    if not args.no_e2e and kind != "u8" and batch == 1 and not nn_lists:
         hs, hd = src.cpu().pin_memory(), dst.cpu().pin_memory()
         hm = [b.cpu().pin_memory() for b in masks]
         hl = torch.empty(n, dtype=torch.int32).pin_memory()
@@ -384,7 +409,7 @@ def run_ours(args):
 
     # ---- config 3 asks for "largest-cluster and wrapping statistics per p": untimed, after the timed region
     statistics = None
-    if rank == 0 and fam in ("triangular", "honeycomb") and kind != "u8":
+    if rank == 0 and fam in ("triangular", "honeycomb") and kind != "u8" and not nn_lists:
         statistics = {}
         wx, wy = ccl.gen_wrap_vectors(fam, size)
         for k, p in enumerate(ps):
@@ -412,7 +437,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": "Gbonds/s", "n_gpus": world, "steps": K,
             "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": text, "calls_per_step": len(ps), "api": "ccl_label_batch" if batch > 1 else "ccl_label" if kind == "u8" else "ccl_label_bits",
+            "config": {"workload": text, "calls_per_step": len(ps), "api": "ccl_label_nn" if nn_lists else "ccl_label_batch" if batch > 1 else "ccl_label" if kind == "u8" else "ccl_label_bits",
                        "parallelism": "replicas x%d (one realization per GPU, no collective)" % world,
                        "l2": "inputs larger than L2 (bond stream %.0f MB per call vs 126 MB L2)" % (stream_bytes / 1e6)
                        if flush is None else "256 MB buffer rewritten between timed calls (L2 flush)",
