@@ -394,3 +394,45 @@ def test_tuning_argument_checks(ccl):
     with pytest.raises(ccl.CclError):
         ccl.set_tuning(0, 12, 5)
     ccl.set_tuning()
+
+
+def test_no_write_outside_the_label_buffer(ccl):
+    """Guard bands around every output buffer stay untouched (compute-sanitizer is not available on the GPU pool)."""
+    rng = np.random.default_rng(404)
+    GUARD, MAGIC = 64, -77
+    for n in (1, 5, 1023, 1024, 1025, 32768, 32769, 100001):
+        m = 3 * n
+        src, dst = graphs.random_graph(rng, n, m, self_loops=True)
+        mask = (rng.random(m) < 0.5).astype(np.uint8)
+        want = oracle.label(n, src, dst, mask)
+        s, d, b = dev(src), dev(dst), bits_dev(graphs.pack_bits(mask))
+
+        def guarded():
+            buf = torch.full((n + 2 * GUARD,), MAGIC, dtype=torch.int32, device="cuda")
+            return buf, buf[GUARD:GUARD + n]
+
+        def intact(buf):
+            return bool((buf[:GUARD] == MAGIC).all().item()) and bool((buf[GUARD + n:] == MAGIC).all().item())
+
+        for opts in ({}, {"two_pass": 1}, {"tile_mode": 1, "small_max_sites": 0}, {"tile_mode": -1},
+                     {"bucket_min_label_bytes": 0, "region_shift": 10, "force_mode": 1}):
+            ccl.set_option("reset")
+            for k, v in opts.items():
+                ccl.set_option(k, v)
+            buf, lab = guarded()
+            if GUARD % 4 == 0:                                  # labels must be 16-byte aligned
+                ccl.label_bits(n, s, d, b, labels=lab)
+                assert intact(buf) and np.array_equal(lab.cpu().numpy(), want), (n, opts)
+        ccl.set_option("reset")
+        buf, lab = guarded()
+        seq, c = ccl.relabel_sequential(dev(want), out=lab)
+        assert intact(buf) and c == int((want == np.arange(n)).sum())
+        if n <= 32768:
+            buf = torch.full((3 * n + 2 * GUARD,), MAGIC, dtype=torch.int32, device="cuda")
+            out = buf[GUARD:GUARD + 3 * n].view(3, n)
+            ccl.label_batch(n, s, d, torch.stack([b, b, b]), 3, labels=out)
+            assert bool((buf[:GUARD] == MAGIC).all().item()) and bool((buf[GUARD + 3 * n:] == MAGIC).all().item())
+            assert np.array_equal(out[2].cpu().numpy(), want)
+        buf, lab = guarded()
+        ccl.label_nn(dev(graphs.nn_list_from_bonds(n, src, dst, mask)), labels=lab)
+        assert intact(buf) and np.array_equal(lab.cpu().numpy(), want)
