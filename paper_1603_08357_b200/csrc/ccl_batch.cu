@@ -30,6 +30,24 @@ __device__ __forceinline__ int32_t smem_root(volatile int32_t* L, int32_t x)
     }
 }
 
+// Analysis (PAPER.md:113 steps (ii)/(iv)) of the forest in shared memory by pointer jumping: every site is re-pointed at
+// its grandparent until nothing changes, about log2(depth) sweeps.  (Walking every chain to its root instead costs the
+// sum of all depths, and hooking raster-ordered lattice sites to their smallest lower neighbour builds long chains.)
+// Must be called by all threads; ends with a barrier.
+__device__ __forceinline__ void smem_flatten(int32_t* L, int32_t n_sites)
+{
+    volatile int32_t* V = L;
+    for (;;) {
+        bool changed = false;
+        for (int32_t i = threadIdx.x; i < n_sites; i += kBatchThreads) {
+            const int32_t p = V[i];
+            const int32_t gp = V[p];
+            if (gp != p) { V[i] = gp; changed = true; }
+        }
+        if (!__syncthreads_or(changed)) return;
+    }
+}
+
 // Steps (i)-(iv) of PAPER.md:113 for realization r = blockIdx.x, all in shared memory:
 //   (i)   L[i] = i, then every occupied bond hooks its higher site to the lower one (one atomicMin, no return value):
 //         each site ends up pointing at its smallest lower-numbered neighbour, the paper's initial label (Fig. 2)
@@ -52,16 +70,7 @@ k_label_batch(int32_t n_sites, int32_t n_bonds, const int32_t* __restrict__ src,
         if (u != v) atomicMin(L + max(u, v), min(u, v));
     }
     __syncthreads();
-    for (int32_t i = tid; i < n_sites; i += kBatchThreads) {
-        int32_t x = i;
-        for (;;) {
-            const int32_t p = reinterpret_cast<volatile int32_t*>(L)[x];
-            if (p == x) break;
-            x = p;
-        }
-        if (x != i) L[i] = x;
-    }
-    __syncthreads();
+    smem_flatten(L, n_sites);
     for (int32_t b = tid; b < n_bonds; b += kBatchThreads) {
         if (occ && !((occ[b >> 5] >> (b & 31)) & 1u)) continue;
         int32_t l1 = src[b], l2 = dst[b];
@@ -76,15 +85,8 @@ k_label_batch(int32_t n_sites, int32_t n_bonds, const int32_t* __restrict__ src,
         }
     }
     __syncthreads();
-    for (int32_t i = tid; i < n_sites; i += kBatchThreads) {
-        int32_t x = L[i];
-        for (;;) {
-            const int32_t p = L[x];
-            if (p == x) break;
-            x = p;
-        }
-        out[i] = x;
-    }
+    smem_flatten(L, n_sites);
+    for (int32_t i = tid; i < n_sites; i += kBatchThreads) out[i] = L[i];
 }
 
 // ---------------------------------------------------------------------------------------- sequential relabel
