@@ -142,6 +142,12 @@ __device__ __forceinline__ uint32_t ld_stream_u8(const uint8_t* p, uint64_t pol)
     return r;
 }
 
+__device__ __forceinline__ void st_stream_pair(int2* p, int2 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.s32 [%0], {%1, %2}, %3;" ::"l"(p), "r"(v.x), "r"(v.y), "l"(pol)
+                 : "memory");
+}
+
 // Label reads during root finding and flattening go through L1 (ld.global.ca).  L1 is not coherent, so a read may
 // return an older value of label[x] -- which is still an ancestor of x, so every walk stays correct and only gets a
 // little longer; every decision that matters is re-validated by the value an atomicMin

@@ -7,12 +7,6 @@
 
 namespace ccl {
 
-__device__ __forceinline__ void st_stream_pair(int2* p, int2 v, uint64_t pol)
-{
-    asm volatile("st.global.L2::cache_hint.v2.s32 [%0], {%1, %2}, %3;" ::"l"(p), "r"(v.x), "r"(v.y), "l"(pol)
-                 : "memory");
-}
-
 // Shared-memory scratch of the CTA-wide append: pairs are counted per target region, one global atomicAdd per
 // region reserves the CTA's range in that bucket, and the pairs leave through a staging array so that consecutive
 // threads write consecutive addresses.
@@ -30,18 +24,6 @@ struct JoinNow {
     int32_t* label;
     __device__ __forceinline__ void operator()(int2 pr) const { algorithm1(label, pr.x, pr.y); }
 };
-// ToList: append to an overflow list that a later kernel works off.
-struct ToList {
-    unsigned long long* count;
-    int2* list;
-    unsigned long long cap;
-    __device__ __forceinline__ void operator()(int2 pr) const
-    {
-        const unsigned long long o = atomicAdd(count, 1ull);
-        if (o < cap) list[o] = pr;
-    }
-};
-
 // Every thread hands in up to P pairs (lo[k] < 0 = none).  Must be called by all THREADS threads of the CTA.
 template <int THREADS, int P, typename Overflow>
 __device__ __forceinline__ void cta_emit(EmitSmem<THREADS, P>& sm, const int32_t (&lo)[P], const int32_t (&hi)[P],

@@ -29,7 +29,6 @@
 // against 0.34-0.40 ms for the 32-way CTA-sorted scatter of ccl_bucket.cu.
 #include "ccl_common.cuh"
 #include "ccl_unionfind.cuh"
-#include "ccl_emit.cuh"
 #include "ccl_bonds.cuh"
 
 namespace ccl {
@@ -37,11 +36,6 @@ namespace ccl {
 constexpr int kTThreads = 1024;                    // k_local, k_small: one CTA per SM
 constexpr int kSThreads = 256;                     // k_scatter_fine
 
-__device__ __forceinline__ void st_pair_stream(int2* p, int2 v, uint64_t pol)
-{
-    asm volatile("st.global.L2::cache_hint.v2.s32 [%0], {%1, %2}, %3;" ::"l"(p), "r"(v.x), "r"(v.y), "l"(pol)
-                 : "memory");
-}
 
 // ------------------------------------------------------------------------------------------ local Algorithm 1
 // Shared-memory window L[0 .. W) holds label[base .. base + W).  Walk x up while its parent stays in the window;
@@ -82,7 +76,7 @@ __device__ __forceinline__ void put_fine(int s, unsigned gpos, int2 pr, TileHead
                                          int2* ovf, unsigned long long cap_o, uint64_t pol)
 {
     if (gpos < cap_f) {
-        st_pair_stream(fine + (size_t)s * cap_f + gpos, pr, pol);
+        st_stream_pair(fine + (size_t)s * cap_f + gpos, pr, pol);
     } else {
         const unsigned long long o = atomicAdd(&hdr->overflow, 1ull);
         if (o < cap_o) ovf[o] = pr;
