@@ -450,6 +450,12 @@ def run_ours(args):
                               "achieved": call_ach, "peak": peak, "unit": "GB/s", "frac": call_ach / peak,
                               "frac_of_8TBs_nominal": call_ach / 8000.0, "bytes_per_call": call_bytes,
                               "avg_call_ms": avg(call_ms)},
+            "roofline_kernels": None if (batch > 1 or nn_lists) else {
+                "k_init (step i)": {"algorithmic_bytes": 4 * n, "avg_ms": avg(init_ms),
+                                    "frac": 4 * n / (avg(init_ms) * 1e-3) / 1e9 / peak},
+                "step (iii)": {"algorithmic_bytes": stream_bytes, "avg_ms": avg(reduce_ms), "frac": ach / peak},
+                "k_flatten (step iv)": {"algorithmic_bytes": 8 * n, "avg_ms": avg(flat_ms),
+                                        "frac": 8 * n / (avg(flat_ms) * 1e-3) / 1e9 / peak}},
             "per_p": per_p, "kernel_ms": {"k_init": avg(init_ms), "k_reduce": avg(reduce_ms), "k_flatten": avg(flat_ms)},
             "statistics": statistics, "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
         }

@@ -59,16 +59,27 @@ k_open_mask(int64_t n_bonds, const uint32_t* __restrict__ bits, const int8_t* __
     }
 }
 
+// Calls f(b, wx, wy) for every occupied bond with a non-zero wrap vector.  The wrap vectors are read 16 bonds at a time
+// (two 128-bit loads, the arrays are 16-byte aligned); on a lattice all but O(L) of the groups are zero and end there.
 template <typename F>
 __device__ __forceinline__ void for_each_occupied_seam_bond(int64_t n_bonds, const uint32_t* __restrict__ bits,
                                                             const int8_t* __restrict__ wx, const int8_t* __restrict__ wy, F f)
 {
+    const int64_t groups = (n_bonds + 15) / 16;
     const int64_t stride = (int64_t)gridDim.x * kWrapThreads;
-    for (int64_t b = (int64_t)blockIdx.x * kWrapThreads + threadIdx.x; b < n_bonds; b += stride) {
-        const int x = wx[b], y = wy[b];
-        if ((x | y) == 0) continue;
-        if (bits && !((bits[b >> 5] >> (b & 31)) & 1u)) continue;
-        f(b, x, y);
+    for (int64_t g = (int64_t)blockIdx.x * kWrapThreads + threadIdx.x; g < groups; g += stride) {
+        const int64_t b0 = g * 16;
+        if (b0 + 16 <= n_bonds) {
+            const int4 a = *reinterpret_cast<const int4*>(wx + b0), c = *reinterpret_cast<const int4*>(wy + b0);
+            if ((a.x | a.y | a.z | a.w | c.x | c.y | c.z | c.w) == 0) continue;
+        }
+        const int64_t b1 = b0 + 16 < n_bonds ? b0 + 16 : n_bonds;
+        for (int64_t b = b0; b < b1; ++b) {
+            const int x = wx[b], y = wy[b];
+            if ((x | y) == 0) continue;
+            if (bits && !((bits[b >> 5] >> (b & 31)) & 1u)) continue;
+            f(b, x, y);
+        }
     }
 }
 
@@ -155,7 +166,7 @@ extern "C" int ccl_wrap(int64_t n_sites, int64_t n_bonds, const int32_t* src, co
     }
     const int rc = ccl_label_bits(n_sites, n_bonds, src, dst, bits_open, labels_open, stream);
     if (rc != CCL_OK || n_bonds == 0) return rc;
-    blocks = (n_bonds + kWrapThreads - 1) / kWrapThreads;
+    blocks = ((n_bonds + 15) / 16 + kWrapThreads - 1) / kWrapThreads;
     if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
     k_wrap_init<<<(unsigned)blocks, kWrapThreads, 0, st>>>(n_bonds, src, dst, occupied_bits, wx, wy, labels_open, node);
     CCL_CHECK_LAUNCH("k_wrap_init");
