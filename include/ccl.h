@@ -167,6 +167,14 @@ int ccl_label_batch(int64_t n_sites, int64_t n_bonds, const int32_t* src, const 
 int ccl_relabel_sequential(int64_t n_sites, const int32_t* labels, int32_t* seq_labels, int64_t* n_clusters,
                            void* workspace, size_t* workspace_bytes, void* stream);
 
+/* An occupancy sweep over ONE bond list with host buffers (BASELINE.json configs 3 and 5 sweep p): the bond list is
+ * copied to the device once, mask k is labeled while the labels of mask k-1 travel back on a second stream.
+ * host_occupied_bits / host_labels: host arrays of n_masks host pointers (a NULL mask = every bond occupied; label
+ * buffers of n_sites int32 each).  Synchronises before returning.  Same results as n_masks ccl_label_bits_host calls. */
+int ccl_label_sweep_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_src, const int32_t* host_dst,
+                         int32_t n_masks, const uint32_t* const* host_occupied_bits, int32_t* const* host_labels,
+                         void* stream);
+
 /* ---- tuning --------------------------------------------------------------------------------------------
  *
  * ccl_set_option(name, value): process-wide knobs; none of them changes the result of ccl_label.  Step (iii) has two

@@ -15,7 +15,7 @@ lib = C.CDLL(_LIB_PATH)
 EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangular", "ccl_gen_honeycomb",
            "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
            "ccl_set_profile_events", "ccl_set_option", "ccl_label_batch", "ccl_relabel_sequential", "ccl_gen_cayley3",
-           "ccl_gen_wrap_vectors", "ccl_wrap", "ccl_label_nn", "ccl_last_error",
+           "ccl_gen_wrap_vectors", "ccl_wrap", "ccl_label_nn", "ccl_label_sweep_host", "ccl_last_error",
            "ccl_version", "ccl_launch_count"]
 
 _vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
@@ -41,7 +41,8 @@ lib.ccl_gen_cayley3.argtypes = [_i32, _vp, _vp, _vp, _vp]
 lib.ccl_gen_wrap_vectors.argtypes = [_i32, _i32, _vp, _vp, _vp]
 lib.ccl_wrap.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
 lib.ccl_label_nn.argtypes = [_i64, _i32, _vp, _vp, _vp]
-for _n in EXPORTS[:17]:
+lib.ccl_label_sweep_host.argtypes = [_i64, _i64, _vp, _vp, _i32, _vp, _vp, _vp]
+for _n in EXPORTS[:18]:
     getattr(lib, _n).restype = C.c_int
 
 
@@ -150,6 +151,17 @@ def label_bits_host(n_sites, src, dst, occupied_bits, labels):
     _check(lib.ccl_label_bits_host(n_sites, src.numel(), _host(src, "src"), _host(dst, "dst"),
                                    _host(occupied_bits, "occupied_bits"), _host(labels, "labels"), _stream()),
            "ccl_label_bits_host")
+    return labels
+
+
+def label_sweep_host(n_sites, src, dst, masks, labels):
+    """ccl_label_sweep_host: HOST tensors; masks / labels are lists of CPU int32 tensors (a mask may be None)."""
+    n = len(masks)
+    assert len(labels) == n
+    mp = (C.c_void_p * n)(*[_host(m, "mask") for m in masks])
+    lp = (C.c_void_p * n)(*[_host(t, "labels") for t in labels])
+    _check(lib.ccl_label_sweep_host(n_sites, src.numel(), _host(src, "src"), _host(dst, "dst"), n, mp, lp, _stream()),
+           "ccl_label_sweep_host")
     return labels
 
 

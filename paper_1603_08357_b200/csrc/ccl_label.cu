@@ -475,3 +475,76 @@ extern "C" int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32
     CCL_CUDA_TRY(cudaStreamSynchronize(st));
     return rc;
 }
+
+// An occupancy sweep over one bond list with HOST buffers: the bond list crosses PCIe once, and the labels of mask k
+// travel back on a second stream while mask k+1 is being labeled (two label buffers on the device).
+extern "C" int ccl_label_sweep_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_src, const int32_t* host_dst,
+                                    int32_t n_masks, const uint32_t* const* host_occupied_bits, int32_t* const* host_labels,
+                                    void* stream)
+{
+    using namespace ccl;
+    CCL_REQUIRE(n_masks >= 0, "n_masks < 0");
+    CCL_REQUIRE(n_masks == 0 || (host_occupied_bits != nullptr && host_labels != nullptr), "mask / label pointer array is NULL");
+    if (n_masks == 0) return CCL_OK;
+    int rc = check_args(n_sites, n_bonds, host_src, host_dst, host_labels[0]);
+    if (rc != CCL_OK) return rc;
+    for (int k = 0; k < n_masks; ++k) CCL_REQUIRE(n_sites == 0 || host_labels[k] != nullptr, "a host_labels entry is NULL");
+    if (n_sites == 0) return CCL_OK;
+    cudaStream_t st = as_stream(stream);
+    const size_t bond_bytes = (size_t)n_bonds * sizeof(int32_t);
+    const size_t mask_bytes = (size_t)((n_bonds + 31) / 32) * sizeof(uint32_t);
+    const size_t label_bytes = (size_t)n_sites * sizeof(int32_t);
+    int32_t *d_src = nullptr, *d_dst = nullptr, *d_labels[2] = {nullptr, nullptr};
+    uint32_t* d_bits[2] = {nullptr, nullptr};
+    cudaStream_t side = nullptr;
+    cudaEvent_t labeled[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+    auto cleanup = [&]() {
+        for (int j = 0; j < 2; ++j) {
+            if (d_bits[j]) cudaFreeAsync(d_bits[j], st);
+            if (d_labels[j]) cudaFreeAsync(d_labels[j], st);
+        }
+        if (d_dst) cudaFreeAsync(d_dst, st);
+        if (d_src) cudaFreeAsync(d_src, st);
+        cudaStreamSynchronize(st);
+        for (int j = 0; j < 2; ++j) { if (labeled[j]) cudaEventDestroy(labeled[j]); if (copied[j]) cudaEventDestroy(copied[j]); }
+        if (side) cudaStreamDestroy(side);
+    };
+#define SWEEP_TRY(expr)                                                                             \
+    do {                                                                                            \
+        cudaError_t e__ = (expr);                                                                   \
+        if (e__ != cudaSuccess) { set_error("%s failed: %s", #expr, cudaGetErrorString(e__)); cleanup(); return CCL_CUDA_ERROR; } \
+    } while (0)
+    SWEEP_TRY(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
+    for (int j = 0; j < 2; ++j) {
+        SWEEP_TRY(cudaEventCreateWithFlags(&labeled[j], cudaEventDisableTiming));
+        SWEEP_TRY(cudaEventCreateWithFlags(&copied[j], cudaEventDisableTiming));
+        if ((rc = scratch_alloc((void**)&d_labels[j], label_bytes, st)) != CCL_OK) { cleanup(); return rc; }
+        if (n_bonds > 0 && (rc = scratch_alloc((void**)&d_bits[j], mask_bytes, st)) != CCL_OK) { cleanup(); return rc; }
+    }
+    if (n_bonds > 0) {
+        if ((rc = scratch_alloc((void**)&d_src, bond_bytes, st)) != CCL_OK) { cleanup(); return rc; }
+        if ((rc = scratch_alloc((void**)&d_dst, bond_bytes, st)) != CCL_OK) { cleanup(); return rc; }
+        SWEEP_TRY(cudaMemcpyAsync(d_src, host_src, bond_bytes, cudaMemcpyHostToDevice, st));
+        SWEEP_TRY(cudaMemcpyAsync(d_dst, host_dst, bond_bytes, cudaMemcpyHostToDevice, st));
+    }
+    for (int k = 0; k < n_masks; ++k) {
+        const int j = k & 1;
+        const uint32_t* bits = nullptr;
+        if (n_bonds > 0 && host_occupied_bits[k] != nullptr) {
+            SWEEP_TRY(cudaMemcpyAsync(d_bits[j], host_occupied_bits[k], mask_bytes, cudaMemcpyHostToDevice, st));
+            bits = d_bits[j];
+        }
+        if (k >= 2) SWEEP_TRY(cudaStreamWaitEvent(st, copied[j], 0));        // label buffer j is free again
+        rc = label_impl(n_sites, n_bonds, d_src, d_dst, bits, 2, d_labels[j], st);
+        if (rc != CCL_OK) { cleanup(); return rc; }
+        SWEEP_TRY(cudaEventRecord(labeled[j], st));
+        SWEEP_TRY(cudaStreamWaitEvent(side, labeled[j], 0));
+        SWEEP_TRY(cudaMemcpyAsync(host_labels[k], d_labels[j], label_bytes, cudaMemcpyDeviceToHost, side));
+        SWEEP_TRY(cudaEventRecord(copied[j], side));
+    }
+    for (int j = 0; j < 2 && j < n_masks; ++j) SWEEP_TRY(cudaStreamWaitEvent(st, copied[j], 0));
+#undef SWEEP_TRY
+    cleanup();                                            // frees in stream order, synchronises, destroys the side stream
+    return CCL_OK;
+}
+

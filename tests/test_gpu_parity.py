@@ -208,6 +208,26 @@ def test_host_buffer_entry_point(ccl):
     assert np.array_equal(out2.numpy(), want)
 
 
+def test_host_buffer_sweep_entry_point(ccl):
+    n, src, dst, ps, cfg = _case("regular4")
+    hs, hd = torch.from_numpy(src).pin_memory(), torch.from_numpy(dst).pin_memory()
+    masks, wants = [], []
+    for r, p in enumerate([0.25, 1 / 3, 0.45, 0.0, 1.0]):
+        mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(cfg), realization=r)
+        masks.append(torch.from_numpy(bits.view(np.int32)).pin_memory())
+        wants.append(oracle.label(n, src, dst, mask))
+    masks.append(None)                                               # no mask: every bond occupied
+    wants.append(oracle.label(n, src, dst))
+    outs = [torch.empty(n, dtype=torch.int32).pin_memory() for _ in masks]
+    ccl.label_sweep_host(n, hs, hd, masks, outs)
+    for got, want in zip(outs, wants):
+        assert np.array_equal(got.numpy(), want)
+    one = [torch.empty(n, dtype=torch.int32)]                        # a single mask, pageable memory
+    ccl.label_sweep_host(n, torch.from_numpy(src), torch.from_numpy(dst), [torch.from_numpy(masks[2].numpy().copy())], one)
+    assert np.array_equal(one[0].numpy(), wants[2])
+    ccl.label_sweep_host(n, hs, hd, [], [])
+
+
 # ------------------------------------------------------------------ region-bucketed form of step (iii)
 @pytest.fixture
 def bucketed(ccl):
