@@ -26,33 +26,6 @@ namespace ccl {
 
 constexpr int kBThreads = 256;
 
-// ---------------------------------------------------------------------------------------------------- probe
-// Samples bonds at a fixed stride and looks at how many join two different regions.  Random numbering: 1 - 1/R of
-// them; raster-ordered lattice: only those on region borders.
-__global__ void __launch_bounds__(1024)
-k_probe(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, int shift, int force_mode,
-        const int32_t* gate, BucketHeader* hdr)
-{
-    __shared__ int s_cross;
-    if (gate != nullptr && *gate == 0) {               // the tiled form (ccl_tile.cu) has done steps (i)-(iii)
-        if (threadIdx.x == 0) hdr->mode = 2;
-        return;
-    }
-    if (threadIdx.x == 0) s_cross = 0;
-    __syncthreads();
-    const int64_t samples = n_bonds < 8192 ? n_bonds : 8192;
-    const int64_t stride = n_bonds / samples;
-    int cross = 0;
-    for (int64_t i = threadIdx.x; i < samples; i += 1024) {
-        const int32_t u = src[i * stride], v = dst[i * stride];
-        cross += (u >> shift) != (v >> shift);
-    }
-    for (int o = 16; o > 0; o >>= 1) cross += __shfl_xor_sync(0xffffffffu, cross, o);
-    if ((threadIdx.x & 31) == 0 && cross) atomicAdd(&s_cross, cross);
-    __syncthreads();
-    if (threadIdx.x == 0) hdr->mode = force_mode >= 0 ? force_mode : ((4 * (int64_t)s_cross >= samples) ? 1 : 0);
-}
-
 // -------------------------------------------------------------------------------------------------- scatter
 // One pass over the bond stream: occupied, non-loop bonds become (lo, hi) pairs filed under region(hi).
 template <int MASK>
@@ -179,9 +152,8 @@ k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long
 }
 
 // ------------------------------------------------------------------------------------------------- host side
-int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                    int mask_kind, int32_t* labels, cudaStream_t st, const int32_t* gate, BucketHeader** hdr_out,
-                    void** ws_out)
+int bucketed_begin(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, cudaStream_t st,
+                   BucketPlan* plan, ProbeJob* job, void** ws_out)
 {
     // region size: 2^23 sites (32 MiB of labels) unless that would need more than kMaxRegions regions
     int shift = tuning().region_shift;
@@ -195,12 +167,28 @@ int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const 
     void* ws = nullptr;
     { const int rc = scratch_alloc(&ws, bytes, st); if (rc != CCL_OK) return rc; }
     *ws_out = ws;
-    BucketHeader* hdr = static_cast<BucketHeader*>(ws);
-    int2* buckets = reinterpret_cast<int2*>(static_cast<char*>(ws) + hdr_bytes);
-    *hdr_out = hdr;
-    CCL_CUDA_TRY(cudaMemsetAsync(hdr, 0, sizeof(BucketHeader), st));
-    k_probe<<<1, 1024, 0, st>>>(n_bonds, src, dst, shift, tuning().force_mode, gate, hdr);
-    CCL_CHECK_LAUNCH("k_probe");
+    plan->hdr = static_cast<BucketHeader*>(ws);
+    plan->buckets = static_cast<char*>(ws) + hdr_bytes;
+    plan->cap = cap;
+    plan->shift = shift;
+    plan->n_regions = n_regions;
+    job->hdr = plan->hdr;
+    job->n_bonds = n_bonds;
+    job->src = src;
+    job->dst = dst;
+    job->shift = shift;
+    job->force_mode = tuning().force_mode;
+    CCL_CUDA_TRY(cudaMemsetAsync(plan->hdr, 0, sizeof(BucketHeader), st));
+    return CCL_OK;
+}
+
+int bucketed_launch(const BucketPlan& plan, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
+                    int mask_kind, int32_t* labels, cudaStream_t st)
+{
+    BucketHeader* hdr = plan.hdr;
+    int2* buckets = static_cast<int2*>(plan.buckets);
+    const unsigned long long cap = plan.cap;
+    const int shift = plan.shift;
     const uintptr_t al = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     const int vec = (al & 15) == 0;
     const int grid = kSMs * 6;
@@ -211,7 +199,7 @@ int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const 
     else
         k_scatter<2><<<grid, kBThreads, 0, st>>>(n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels);
     CCL_CHECK_LAUNCH("k_scatter");
-    for (int r = n_regions - 1; r >= 0; --r) {
+    for (int r = plan.n_regions - 1; r >= 0; --r) {
         k_descend<4><<<grid, kBThreads, 0, st>>>(r, shift, hdr, buckets, cap, labels);
         CCL_CHECK_LAUNCH("k_descend");
     }

@@ -51,7 +51,7 @@ inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s
 constexpr int kMaxRegions = 32;
 
 struct BucketHeader {                              // lives in device memory at the head of the call's workspace
-    int32_t mode;                                  // written by k_probe: 0 = direct one-pass kernel, 1 = bucketed
+    int32_t mode;                                  // written by probe_regions: 0 = direct kernel, 1 = bucketed, 2 = nothing
     int32_t pad;
     unsigned long long count[kMaxRegions];         // pairs filed under each region (may exceed the capacity: the
                                                    // excess was joined on the spot by the general algorithm)
@@ -91,10 +91,29 @@ int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st);
 
 // Enqueues probe + scatter + one descend launch per region.  *ws_out is a cudaMallocAsync allocation the caller
 // frees (cudaFreeAsync) after the kernels that read *hdr_out have been enqueued.
-// gate (may be NULL): device flag; if *gate == 0 the tiled form has done the work and the probe sets mode 2 (nothing).
-int bucketed_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                    int mask_kind, int32_t* labels, cudaStream_t st, const int32_t* gate, BucketHeader** hdr_out,
-                    void** ws_out);
+// The region-bucketed form in two halves, so that its probe can ride in k_init (one block of k_init samples the bond
+// list while the others write label[i] = i; as a kernel of its own the probe was 12 us of pure latency on the critical
+// path of every call).  bucketed_begin allocates and clears the workspace and fills in the probe job;
+// bucketed_launch enqueues the scatter and one descend launch per region.  *ws_out is a cudaMallocAsync allocation the
+// caller frees (cudaFreeAsync) after the kernels that read the header have been enqueued.
+struct ProbeJob {
+    BucketHeader* hdr = nullptr;                   // NULL: no probe
+    int64_t n_bonds = 0;
+    const int32_t* src = nullptr;
+    const int32_t* dst = nullptr;
+    int shift = 0;
+    int force_mode = -1;
+};
+struct BucketPlan {
+    BucketHeader* hdr = nullptr;
+    void* buckets = nullptr;
+    unsigned long long cap = 0;
+    int shift = 0, n_regions = 0;
+};
+int bucketed_begin(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, cudaStream_t st,
+                   BucketPlan* plan, ProbeJob* job, void** ws_out);
+int bucketed_launch(const BucketPlan& plan, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
+                    int mask_kind, int32_t* labels, cudaStream_t st);
 
 // Tiled form of steps (i)-(iii) for bond lists that are local in the site numbering (ccl_tile.cu).  *done says what
 // was enqueued: kTiledNo nothing (call outside its range); kTiledFinal labels are final (one-CTA kernel); kTiledIfLocal
@@ -146,6 +165,30 @@ __device__ __forceinline__ void st_stream_pair(int2* p, int2 v, uint64_t pol)
 {
     asm volatile("st.global.L2::cache_hint.v2.s32 [%0], {%1, %2}, %3;" ::"l"(p), "r"(v.x), "r"(v.y), "l"(pol)
                  : "memory");
+}
+
+// Samples up to 8192 bonds at a fixed stride and looks at how many join two different regions (random numbering: 1 - 1/R of
+// them; raster-ordered lattice: only those on region borders): mode 1 = region-bucketed form, 0 = direct kernel.  Called
+// by all threads of ONE block; gated = another form has done the work (mode 2: nothing to do).
+__device__ __forceinline__ void probe_regions(const ProbeJob& job, bool gated)
+{
+    __shared__ int s_cross;
+    if (gated) { if (threadIdx.x == 0) job.hdr->mode = 2; return; }
+    if (threadIdx.x == 0) s_cross = 0;
+    __syncthreads();
+    const int64_t samples = job.n_bonds < 8192 ? job.n_bonds : 8192;
+    const int64_t stride = job.n_bonds / samples;
+    int cross = 0;
+#pragma unroll 8
+    for (int64_t i = threadIdx.x; i < samples; i += blockDim.x) {
+        const int32_t u = job.src[i * stride], v = job.dst[i * stride];
+        cross += (u >> job.shift) != (v >> job.shift);
+    }
+    for (int o = 16; o > 0; o >>= 1) cross += __shfl_xor_sync(0xffffffffu, cross, o);
+    if ((threadIdx.x & 31) == 0 && cross) atomicAdd(&s_cross, cross);
+    __syncthreads();
+    if (threadIdx.x == 0)
+        job.hdr->mode = job.force_mode >= 0 ? job.force_mode : ((4 * (int64_t)s_cross >= samples) ? 1 : 0);
 }
 
 // Label reads during root finding and flattening go through L1 (ld.global.ca).  L1 is not coherent, so a read may

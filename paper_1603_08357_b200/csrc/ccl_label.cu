@@ -17,9 +17,13 @@ namespace ccl {
 constexpr int kThreads = 256;
 
 // ------------------------------------------------------------------------------------------------ step (i)
-__global__ void __launch_bounds__(kThreads) k_init(int64_t n_sites, int32_t* __restrict__ label, const int32_t* gate)
+__global__ void __launch_bounds__(kThreads)
+k_init(int64_t n_sites, int32_t* __restrict__ label, const int32_t* gate, ProbeJob job)
 {
-    if (gate != nullptr && *gate == 0) return;             // the tiled form (ccl_tile.cu) has written every label
+    const bool gated = gate != nullptr && *gate == 0;      // the tiled form (ccl_tile.cu) has written every label
+    // the probe of the region-bucketed form rides along in block 0, which starts first (ccl_common.cuh)
+    if (job.hdr != nullptr && blockIdx.x == 0) probe_regions(job, gated);
+    if (gated) return;
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
     for (int64_t i = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; i < n_sites; i += stride) {
         if (i + 4 <= n_sites) {
@@ -358,23 +362,31 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
     if (rc != CCL_OK) return rc;
     auto done = [&](int code) { if (tile_ws) cudaFreeAsync(tile_ws, st); return code; };
     if (tiled == kTiledFinal) { mark(0, st); mark(1, st); mark(2, st); return CCL_OK; }
+    void* bucket_ws = nullptr;
+    BucketPlan plan;
+    ProbeJob job;
+    auto done2 = [&](int code) { if (bucket_ws) cudaFreeAsync(bucket_ws, st); return done(code); };
     if (tiled != kTiledForced) {
+        // Label arrays that cannot stay in L2 get the region-bucketed form if a device-side probe finds the bonds
+        // non-local in the site numbering; the direct kernel then returns at once (and vice versa).
+        if (n_bonds > 0 && tuning().force_mode != 0 && n_sites * (int64_t)sizeof(int32_t) >= tuning().bucket_min_label_bytes &&
+            n_bonds >= tuning().bucket_min_bonds) {
+            rc = bucketed_begin(n_sites, n_bonds, src, dst, st, &plan, &job, &bucket_ws);
+            if (rc != CCL_OK) return done2(rc);
+        }
         const int64_t init_blocks = site_blocks < (int64_t)kSMs * 32 ? site_blocks : (int64_t)kSMs * 32;
-        k_init<<<(unsigned)init_blocks, kThreads, 0, st>>>(n_sites, labels, gate);              // step (i)
-        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_init failed: %s", cudaGetErrorString(e)); return done(CCL_CUDA_ERROR); } count_launch(); }
+        k_init<<<(unsigned)init_blocks, kThreads, 0, st>>>(n_sites, labels, gate, job);         // step (i) (+ the probe)
+        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_init failed: %s", cudaGetErrorString(e)); return done2(CCL_CUDA_ERROR); } count_launch(); }
     }
     // step (ii): nothing to do after label[i] = i (every site is a root).
     mark(0, st);
     if (n_bonds > 0) {
         if (tiled != kTiledForced) {
-            // step (iii).  Label arrays that cannot stay in L2 get the region-bucketed form if a device-side probe finds
-            // the bonds non-local in the site numbering; the direct kernel then returns at once (and vice versa).
-            BucketHeader* hdr = nullptr;
-            void* ws = nullptr;
-            if (tuning().force_mode != 0 && n_sites * (int64_t)sizeof(int32_t) >= tuning().bucket_min_label_bytes &&
-                n_bonds >= tuning().bucket_min_bonds) {
-                rc = bucketed_reduce(n_sites, n_bonds, src, dst, occ, mask_kind, labels, st, gate, &hdr, &ws);
-                if (rc != CCL_OK) { if (ws) cudaFreeAsync(ws, st); return done(rc); }
+            // step (iii)
+            BucketHeader* hdr = plan.hdr;
+            if (hdr != nullptr) {
+                rc = bucketed_launch(plan, n_bonds, src, dst, occ, mask_kind, labels, st);
+                if (rc != CCL_OK) return done2(rc);
             }
             // Two passes pay where most bonds close cycles (many bonds per site: triangular lattice 0.70 -> 0.53 ms);
             // with 1.5-2 bonds per site (honeycomb, random regular graphs) they are neutral or slower.
@@ -387,14 +399,14 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
             } else if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, hdr, gate, st);
             else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, hdr, gate, st);
             else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, hdr, gate, st);
-            if (ws) cudaFreeAsync(ws, st);
-            if (rc != CCL_OK) return done(rc);
+            if (rc != CCL_OK) return done2(rc);
         }
         mark(1, st);
         k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels);                 // step (iv)
-        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_flatten failed: %s", cudaGetErrorString(e)); return done(CCL_CUDA_ERROR); } count_launch(); }
+        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_flatten failed: %s", cudaGetErrorString(e)); return done2(CCL_CUDA_ERROR); } count_launch(); }
         mark(2, st);
     }
+    if (bucket_ws) cudaFreeAsync(bucket_ws, st);
     if (tile_ws) cudaFreeAsync(tile_ws, st);
     return CCL_OK;
 }
