@@ -50,7 +50,7 @@ int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st)
 }  // namespace ccl
 
 extern "C" const char* ccl_last_error(void) { return ccl::g_error; }
-extern "C" int ccl_version(void) { return 100; }      // 0.1.0
+extern "C" int ccl_version(void) { return 200; }      // 0.2.0: + label_nn, label_batch, label_sweep_host, relabel, wrap
 extern "C" int64_t ccl_launch_count(void) { return ccl::g_launches; }
 
 extern "C" int ccl_set_option(const char* name, int64_t value)
