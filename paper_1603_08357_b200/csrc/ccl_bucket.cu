@@ -36,6 +36,7 @@ k_scatter(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __res
 {
     constexpr int P = 8;
     __shared__ EmitSmem<kBThreads, P> sm;
+    pdl_wait();
     if (hdr->mode != 1) return;
     const uint64_t pol = evict_first_policy();
     const int64_t tiles = (n_bonds + kBThreads * P - 1) / (kBThreads * P);
@@ -85,6 +86,7 @@ __global__ void __launch_bounds__(kBThreads)
 k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long cap, int32_t* label)
 {
     __shared__ EmitSmem<kBThreads, P> sm;
+    pdl_wait();
     if (hdr->mode != 1) return;
     const uint64_t pol = evict_first_policy();
     unsigned long long n = hdr->count[r];
@@ -149,6 +151,7 @@ k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long
         for (int k = 0; k < P; ++k) if (!pend[k]) a[k] = -1;
         cta_emit<kBThreads, P>(sm, a, b, shift, hdr, buckets, cap, JoinNow{label}, pol);
     }
+    pdl_go();                                              // this CTA is done: the next launch may take its place
 }
 
 // ------------------------------------------------------------------------------------------------- host side
@@ -193,15 +196,15 @@ int bucketed_launch(const BucketPlan& plan, int64_t n_bonds, const int32_t* src,
     const int vec = (al & 15) == 0;
     const int grid = kSMs * 6;
     if (occ == nullptr)
-        k_scatter<0><<<grid, kBThreads, 0, st>>>(n_bonds, src, dst, nullptr, vec, shift, hdr, buckets, cap, labels);
+        CCL_CUDA_TRY(launch_pdl(k_scatter<0>, (unsigned)grid, (unsigned)kBThreads, st, n_bonds, src, dst, (const void*)nullptr, vec, shift, hdr, buckets, cap, labels));
     else if (mask_kind == 1)
-        k_scatter<1><<<grid, kBThreads, 0, st>>>(n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels);
+        CCL_CUDA_TRY(launch_pdl(k_scatter<1>, (unsigned)grid, (unsigned)kBThreads, st, n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels));
     else
-        k_scatter<2><<<grid, kBThreads, 0, st>>>(n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels);
-    CCL_CHECK_LAUNCH("k_scatter");
+        CCL_CUDA_TRY(launch_pdl(k_scatter<2>, (unsigned)grid, (unsigned)kBThreads, st, n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels));
+    count_launch();
     for (int r = plan.n_regions - 1; r >= 0; --r) {
-        k_descend<4><<<grid, kBThreads, 0, st>>>(r, shift, hdr, buckets, cap, labels);
-        CCL_CHECK_LAUNCH("k_descend");
+        CCL_CUDA_TRY(launch_pdl(k_descend<4>, (unsigned)grid, (unsigned)kBThreads, st, r, shift, hdr, buckets, cap, labels));
+        count_launch();
     }
     return CCL_OK;
 }

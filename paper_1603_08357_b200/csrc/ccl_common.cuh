@@ -47,6 +47,31 @@ inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s
         }                                                                                          \
     } while (0)
 
+// ---- programmatic dependent launch -----------------------------------------------------------------------
+// A kernel launched with launch_pdl may be scheduled while its predecessor on the stream is still draining; it calls
+// pdl_wait() before it touches anything the predecessor wrote (the wait returns when the predecessor has completed and
+// its writes are visible), and pdl_go() early, to let its own successor be scheduled the same way.  This hides the
+// launch latency between the kernels of one call (a dozen short launches on config 5).  Both calls are no-ops in a
+// kernel that was launched the ordinary way.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_go() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... Params, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(Params...), unsigned grid, unsigned block, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
+}
+
 // ---- region-bucketed label reduction (ccl_bucket.cu) -----------------------------------------------------
 constexpr int kMaxRegions = 32;
 

@@ -114,6 +114,7 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
          const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
 {
     __shared__ int2 queue[kThreads / 32][128];
+    pdl_wait();
     if (hdr != nullptr && hdr->mode != 0) return;          // the bucketed form (ccl_bucket.cu) did step (iii)
     if (gate != nullptr && *gate == 0) return;             // the tiled form (ccl_tile.cu) did
     const uint64_t pol = evict_first_policy();
@@ -155,6 +156,7 @@ __global__ void __launch_bounds__(kThreads)
 k_hook(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, const void* __restrict__ occ,
        int vec, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
 {
+    pdl_wait();
     if ((hdr != nullptr && hdr->mode != 0) || (gate != nullptr && *gate == 0)) return;      // another form did step (iii)
     const uint64_t pol = evict_first_policy();
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
@@ -172,6 +174,7 @@ k_join(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restri
        int vec, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
 {
     __shared__ int2 queue[kThreads / 32][128];
+    pdl_wait();
     if ((hdr != nullptr && hdr->mode != 0) || (gate != nullptr && *gate == 0)) return;
     const uint64_t pol = evict_first_policy();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -216,8 +219,9 @@ k_join(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restri
 // writers only ever replace a chain pointer by the root of the same chain, so a reader sees either and still
 // arrives at the root.  Roots and already-flat sites are not rewritten.
 __global__ void __launch_bounds__(kThreads)
-k_flatten(int64_t n_sites, int32_t* label, const BucketHeader* hdr = nullptr, const int32_t* gate = nullptr)
+k_flatten(int64_t n_sites, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
 {
+    pdl_wait();
     if ((hdr != nullptr && hdr->mode != 0) || (gate != nullptr && *gate == 0)) return;      // only for the mid-call flatten
     const int64_t i0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
     if (i0 >= n_sites) return;
@@ -294,9 +298,9 @@ static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst
         set_error("invalid argument: occupied_bits is not 4-byte aligned");
         return CCL_INVALID_ARG;
     }
-    if (vec) k_reduce<MASK, true><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels, hdr, gate);
-    else     k_reduce<MASK, false><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, labels, hdr, gate);
-    CCL_CHECK_LAUNCH("k_reduce");
+    if (vec) CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, true>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate));
+    else     CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, false>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate));
+    count_launch();
     return CCL_OK;
 }
 
@@ -315,12 +319,12 @@ static int launch_two_pass(int64_t n_sites, int64_t n_bonds, const int32_t* src,
         return CCL_INVALID_ARG;
     }
     const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
-    k_hook<MASK><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, vec, labels, hdr, gate);     // step (i), paper form
-    CCL_CHECK_LAUNCH("k_hook");
-    k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels, hdr, gate);                      // step (ii)
-    CCL_CHECK_LAUNCH("k_flatten");
-    k_join<MASK><<<(unsigned)blocks, kThreads, 0, st>>>(n_bonds, src, dst, occ, vec, labels, hdr, gate);     // step (iii)
-    CCL_CHECK_LAUNCH("k_join");
+    CCL_CUDA_TRY(launch_pdl(k_hook<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, gate));   // step (i), paper form
+    count_launch();
+    CCL_CUDA_TRY(launch_pdl(k_flatten, (unsigned)site_blocks, (unsigned)kThreads, st, n_sites, labels, hdr, gate));                   // step (ii)
+    count_launch();
+    CCL_CUDA_TRY(launch_pdl(k_join<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, gate));   // step (iii)
+    count_launch();
     return CCL_OK;
 }
 
@@ -328,7 +332,7 @@ static int launch_two_pass(int64_t n_sites, int64_t n_bonds, const int32_t* src,
 int flatten_labels(int64_t n_sites, int32_t* labels, cudaStream_t st)
 {
     const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
-    k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels);
+    k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels, nullptr, nullptr);
     CCL_CHECK_LAUNCH("k_flatten");
     return CCL_OK;
 }
@@ -402,8 +406,12 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
             if (rc != CCL_OK) return done2(rc);
         }
         mark(1, st);
-        k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels);                 // step (iv)
-        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_flatten failed: %s", cudaGetErrorString(e)); return done2(CCL_CUDA_ERROR); } count_launch(); }
+        {                                                                                       // step (iv)
+            const cudaError_t e = launch_pdl(k_flatten, (unsigned)site_blocks, (unsigned)kThreads, st, n_sites, labels,
+                                             (const BucketHeader*)nullptr, (const int32_t*)nullptr);
+            if (e != cudaSuccess) { set_error("launch of k_flatten failed: %s", cudaGetErrorString(e)); return done2(CCL_CUDA_ERROR); }
+            count_launch();
+        }
         mark(2, st);
     }
     if (bucket_ws) cudaFreeAsync(bucket_ws, st);
