@@ -333,7 +333,7 @@ def run_ours(args):
             if flush is not None:
                 flush.fill_(c & 0xFF)
             e = ev[c]
-            if batch > 1 or nn_lists:                 # no per-step events on these entry points
+            if batch > 1 or nn_lists or args.no_kernel_split:   # no per-step events inside the call
                 e[0].record(); e[1].record()
                 one_call(k)
                 e[2].record(); e[3].record()
@@ -486,6 +486,9 @@ def main():
     ap.add_argument("--force-mode", type=int, default=-1, help="experiment: -1 probe, 0 direct, 1 bucketed")
     ap.add_argument("--option", action="append", default=[], help="experiment: name=value for ccl_set_option")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-kernel-split", action="store_true",
+                    help="do not record events between the kernels of a call (an event record between two kernels keeps them "
+                         "from overlapping by programmatic dependent launch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
