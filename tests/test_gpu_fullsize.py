@@ -63,3 +63,40 @@ def test_cfg5_regular4_2p26(ccl):
     d_src, d_dst = ccl.gen_regular(n, 4, oracle.seed_for(5))
     torch.cuda.empty_cache()
     _check(ccl, n, src, dst, d_src, d_dst, [0.25, 1.0 / 3.0, 0.45], 5)
+
+
+def test_maximum_site_count(ccl):
+    """n_sites = 2^31 - 1 (the largest the int32 labels allow): 4 M random bonds over the whole range plus a few placed at
+    the very ends.  Expected labels of the touched sites come from the oracle on the order-preserving compaction of the
+    touched sites (the smallest site of a component stays the smallest); every other site must be its own label."""
+    n = (1 << 31) - 1
+    rng = np.random.default_rng(2031)
+    m = 1 << 22
+    src = rng.integers(0, n, size=m, dtype=np.int64)
+    dst = rng.integers(0, n, size=m, dtype=np.int64)
+    src[:6] = [0, n - 2, 5, n - 1, 1 << 30, (1 << 30) + 1]
+    dst[:6] = [n - 1, n - 1, 7, 12345, (1 << 30) - 1, n - 3]
+    mask = (rng.random(m) < 0.8).astype(np.uint8)
+    mask[:6] = 1
+    touched, inv = np.unique(np.concatenate([src, dst]), return_inverse=True)
+    csrc, cdst = inv[:m].astype(np.int32), inv[m:].astype(np.int32)
+    want_compact = oracle.label(touched.size, csrc, cdst, mask)
+    want = touched[want_compact]                                        # expected label of site touched[k]
+    s = torch.from_numpy(src.astype(np.int32)).cuda()
+    d = torch.from_numpy(dst.astype(np.int32)).cuda()
+    for form in ("u8", "bits"):
+        if form == "u8":
+            lab = ccl.label(n, s, d, torch.from_numpy(mask).cuda())
+        else:
+            import graphs
+            lab = ccl.label_bits(n, s, d, torch.from_numpy(graphs.pack_bits(mask).view(np.int32)).cuda())
+        got = lab[torch.from_numpy(touched).cuda()].cpu().numpy().astype(np.int64)
+        assert np.array_equal(got, want)
+        moved = 0                                                      # sites whose label is not their own index
+        step = 1 << 28
+        for lo in range(0, n, step):
+            hi = min(n, lo + step)
+            moved += int((lab[lo:hi] != torch.arange(lo, hi, dtype=torch.int32, device="cuda")).sum().item())
+        assert moved == int((want != touched).sum())
+        del lab
+        torch.cuda.empty_cache()
