@@ -173,3 +173,27 @@ def test_wrapping_detection_larger_lattices(ccl, family, L):
         row[3 * np.arange(5 * L, 6 * L)] = 1                # bonds k = 0 of row y = 5
         got = ccl.wrap(n, s, d, torch.from_numpy(graphs.pack_bits(row).view(np.int32)).cuda(), gx, gy)[:2]
         assert got == (True, False) == oracle.wrap(n, src, dst, dx, dy, row)
+
+
+@pytest.mark.parametrize("family", ["triangular", "honeycomb"])
+def test_wrapping_detection_with_reversed_bonds(ccl, family):
+    """A bond listed the other way round carries the negated wrap vector (-1 entries); the answer must not change."""
+    pc = 0.3473 if family == "triangular" else 0.6527
+    rng = np.random.default_rng(17)
+    for L in (4, 9, 33, 64):
+        src, dst, dx, dy, wx, wy = _wrap_vectors_from_oracle(family, L)
+        n = (2 if family == "honeycomb" else 1) * L * L
+        flip = rng.random(src.size) < 0.5
+        s2 = np.where(flip, dst, src).astype(np.int32)
+        d2 = np.where(flip, src, dst).astype(np.int32)
+        wx2 = np.where(flip, -wx, wx).astype(np.int8)
+        wy2 = np.where(flip, -wy, wy).astype(np.int8)
+        perm = rng.permutation(src.size)                    # and in any bond order
+        for r in range(30):
+            mask, _ = oracle.gen_occupancy(src.size, pc + 0.04 * (r % 5 - 2), oracle.seed_for(3), realization=200 + r)
+            want = oracle.wrap(n, src, dst, dx, dy, mask)
+            bits = graphs.pack_bits(mask[perm])
+            got = ccl.wrap(n, torch.from_numpy(s2[perm]).cuda(), torch.from_numpy(d2[perm]).cuda(),
+                           torch.from_numpy(bits.view(np.int32)).cuda(), torch.from_numpy(wx2[perm]).cuda(),
+                           torch.from_numpy(wy2[perm]).cuda())[:2]
+            assert got == want, (L, r)
