@@ -197,3 +197,29 @@ def test_wrapping_detection_with_reversed_bonds(ccl, family):
                            torch.from_numpy(bits.view(np.int32)).cuda(), torch.from_numpy(wx2[perm]).cuda(),
                            torch.from_numpy(wy2[perm]).cuda())[:2]
             assert got == want, (L, r)
+
+
+@pytest.mark.parametrize("family,pc", [("triangular", 0.34729635533386066), ("honeycomb", 0.6527036446661394)])
+def test_wrapping_probability_curves_cross_at_the_exact_threshold(ccl, family, pc):
+    """The paper's own correctness evidence (Figs. 5-6): the spanning-probability curves of different
+    sizes cross at p_c.  Here through the CUDA path alone (device generators, ccl_wrap), 400 realizations per point:
+    below p_c the larger lattice wraps less often, above p_c more often, and at p_c the two agree."""
+    reals = 400
+    R = {}
+    for L in (24, 72):
+        src, dst = (ccl.gen_triangular if family == "triangular" else ccl.gen_honeycomb)(L)
+        wx, wy = ccl.gen_wrap_vectors(family, L)
+        n = (2 if family == "honeycomb" else 1) * L * L
+        lab = torch.empty(n, dtype=torch.int32, device="cuda")
+        for p in (pc - 0.02, pc, pc + 0.02):
+            hits = 0
+            for r in range(reals):
+                _, bits = ccl.gen_occupancy(3 * L * L, p, oracle.seed_for(3) + L, r, want_mask=False)
+                x, y, _ = ccl.wrap(n, src, dst, bits, wx, wy, labels_open=lab)
+                hits += x or y
+            R[(L, p)] = hits / reals
+    lo, hi = pc - 0.02, pc + 0.02
+    assert R[(72, lo)] < R[(24, lo)] - 0.08, R             # curves fan out on both sides ...
+    assert R[(72, hi)] > R[(24, hi)] + 0.03, R
+    assert abs(R[(72, pc)] - R[(24, pc)]) < 0.12, R        # ... and meet at the exact threshold (4 sigma of 400 draws)
+    assert 0.5 < R[(24, pc)] < 0.85 and 0.5 < R[(72, pc)] < 0.85, R      # SURVEY 8(c): R_either ~ 0.68-0.69 at p_c
