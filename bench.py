@@ -49,7 +49,7 @@ def describe(name):
     fam, size, z, ps, kind, cfg = WORKLOADS[name]
     if fam == "regular":
         n, m = size, size * z // 2
-        text = "cfg%d random %d-regular N=2^%d M=%d" % (cfg, z, size.bit_length() - 1, m)
+        text = "%s random %d-regular N=%d M=%d" % ("cfg%d" % cfg if cfg < 9 else "custom", z, size, m)
     elif fam == "cayley":
         n = 3 * (1 << size) - 2
         m = n - 1
@@ -63,7 +63,7 @@ def describe(name):
     else:
         n = (2 if fam == "honeycomb" else 1) * size * size
         m = 3 * size * size
-        text = "cfg%d %s L=%d periodic N=%d M=%d" % (cfg, fam, size, n, m)
+        text = "%s %s L=%d periodic N=%d M=%d" % ("cfg%d" % cfg if cfg < 9 else "custom", fam, size, n, m)
     return n, m, text + " p=" + ",".join("%.4g" % p for p in ps) + " mask=" + kind
 
 
@@ -482,6 +482,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--family", choices=["triangular", "honeycomb", "regular", "cayley"],
+                    help="a workload outside the table: --family with --size (L, or sites for regular, or generations for "
+                         "cayley), --z (degree; cayley: 1 = random numbering) and --p (comma-separated); used for the "
+                         "paper's own sizes (PAPER.md:171-173, 193)")
+    ap.add_argument("--size", type=int, default=0)
+    ap.add_argument("--z", type=int, default=0)
+    ap.add_argument("--p", default="")
     ap.add_argument("--region-shift", type=int, default=-1, help="experiment: log2 sites per region of the bucketed form")
     ap.add_argument("--force-mode", type=int, default=-1, help="experiment: -1 probe, 0 direct, 1 bucketed")
     ap.add_argument("--option", action="append", default=[], help="experiment: name=value for ccl_set_option")
@@ -491,6 +498,12 @@ def main():
                          "from overlapping by programmatic dependent launch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.family:
+        ps = [float(t) for t in args.p.split(",") if t]
+        if not ps or args.size <= 0:
+            ap.error("--family needs --size and --p")
+        WORKLOADS["custom"] = (args.family, args.size, args.z, ps, "bits", 9)
+        args.workload = "custom"
     if args.impl == "reference":
         run_reference(args)
     else:
