@@ -12,8 +12,12 @@
  * Conventions for every entry point
  *   - All array pointers are DEVICE pointers owned by the caller unless the name says `host_`.  The library
  *     never frees caller memory.  Scratch a call needs comes from the library's own stream-ordered memory pool
- *     (cudaMallocFromPoolAsync) and is returned to that pool, in stream order, before the call returns; the pool
- *     keeps the memory for the next call.
+ *     (one cudaMemPool_t per device, cudaMallocFromPoolAsync) and is returned to that pool, in stream order, before
+ *     the call returns.  The pool KEEPS what it has reserved for the next call (so that a sweep of calls does not
+ *     pay the driver for memory each time) until ccl_trim_scratch() hands it back; ccl_scratch_bytes() reports it.
+ *     What a call draws: ccl_label / ccl_label_bits nothing, unless n_sites * 4 >= 96 MiB and n_bonds >= 2^20 (the
+ *     region-bucketed form): then 10 * n_bonds bytes of pair chunks plus a table (about 1.3 GB for 2^27 bonds);
+ *     the host-buffer entry points also their device copies of src, dst, masks and labels.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the default stream).  All work is enqueued on it; no
  *     entry point synchronises with the host unless stated.  Results are valid once the stream has drained.
  *   - Return value: CCL_OK (0) or a ccl_status.  No exception crosses the ABI.  ccl_last_error() returns a
@@ -51,23 +55,27 @@ typedef struct ccl_stats {
  * ccl_label: bonds b = 0..n_bonds-1 join sites src[b] and dst[b] (two separate int32 arrays); bond b is
  * occupied iff occupied[b] != 0 (one uint8 per bond); occupied == NULL means every bond is occupied.
  * labels[n_sites] (int32) is write-only on entry -- no initial content is required -- and holds the canonical
- * labels on completion.  src, dst, occupied are read-only.  0 <= src[b], dst[b] < n_sites is a caller
+ * labels on completion; it must be 16-byte aligned (else CCL_INVALID_ARG; every cudaMalloc / torch allocation is).
+ * src, dst, occupied are read-only and may have any alignment (16-byte aligned src/dst take the vectorised path).  0 <= src[b], dst[b] < n_sites is a caller
  * precondition that is NOT checked here (use ccl_validate_bonds).  Self-loops and repeated bonds are legal.
  * n_bonds == 0 gives labels[i] = i.  n_sites == 0 is a no-op.  The result does not depend on bond order.
- * Errors: n_sites < 0, n_sites > 2^31-1, n_bonds < 0, or NULL src/dst/labels with a non-zero count
- * -> CCL_INVALID_ARG.
+ * Errors: n_sites < 0, n_sites > 2^31-1, n_bonds < 0, NULL src/dst/labels with a non-zero count, or misaligned
+ * labels -> CCL_INVALID_ARG.
+ * The library remembers, per host thread, what its device-side probe said about the last few bond lists (keyed by
+ * the src/dst pointers and the counts) and skips the probe on later calls; this changes speed only, never results.
  */
 int ccl_label(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
               const uint8_t* occupied, int32_t* labels, void* stream);
 
-/* Same with a packed mask: bond b is bit (b & 31) of uint32 word (b >> 5); ceil(n_bonds/32) words, bits past
- * n_bonds are ignored.  src and dst should be 16-byte aligned for the vectorised path (any alignment works). */
+/* Same with a packed mask: bond b is bit (b & 31) of uint32 word (b >> 5); ceil(n_bonds/32) words (4-byte aligned),
+ * bits past n_bonds are ignored. */
 int ccl_label_bits(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
                    const uint32_t* occupied_bits, int32_t* labels, void* stream);
 
 /* The paper's own interface: a nearest-neighbour list instead of a bond list.  nn_list is a dense
  * z_max x n_sites int32 array, structure of arrays: the k-th neighbour of site i is nn_list[k * n_sites + i]; negative
- * entries are padding.  Every entry is a connection of the network to be labeled (list it from one side or from both).
+ * entries are padding.  Every entry is a connection of the network to be labeled; a bond may be listed at both of its
+ * ends (the paper's form) or at either one.
  * The four steps run in the paper's form: (i) label[i] = smallest lower-numbered neighbour, else i; (ii) analysis;
  * (iii) Algorithm 1 over every (site, lower-numbered neighbour); (iv) analysis.  Same result as ccl_label on the
  * corresponding bond list.  0 <= z_max <= 1024; neighbours >= n_sites are a caller error (not checked). */
@@ -175,25 +183,36 @@ int ccl_label_sweep_host(int64_t n_sites, int64_t n_bonds, const int32_t* host_s
                          int32_t n_masks, const uint32_t* const* host_occupied_bits, int32_t* const* host_labels,
                          void* stream);
 
+/* ---- scratch memory ---------------------------------------------------------------------------------------
+ *
+ * ccl_trim_scratch: synchronises `stream`, then returns to the driver all memory the library's pool on the current
+ * device holds beyond keep_bytes (0 = everything that is not in use).  ccl_scratch_bytes: bytes the pool has
+ * reserved from the driver / bytes currently handed out to calls in flight (either pointer may be NULL; host pointers). */
+int ccl_trim_scratch(size_t keep_bytes, void* stream);
+int ccl_scratch_bytes(int64_t* reserved, int64_t* in_use);
+
 /* ---- tuning --------------------------------------------------------------------------------------------
  *
- * ccl_set_option(name, value): process-wide knobs; none of them changes the result of ccl_label.  Step (iii) has two
- * forms: the direct one-pass kernel, and a region-bucketed form for label arrays too large for
- * L2, which a device-side probe selects when the bonds are not local in the site numbering.
+ * ccl_set_option(name, value): knobs of the CALLING HOST THREAD (like ccl_last_error and ccl_launch_count; a call
+ * reads them once on entry, so another thread can never change a call in flight); none of them changes the result of
+ * ccl_label.  Step (iii) has two forms: the direct kernels, and a region-bucketed form for label
+ * arrays too large for L2, which a device-side probe selects when the bonds are not local in the site numbering.
  *   "bucket_min_label_bytes"  label arrays of at least this many bytes are eligible for the bucketed form
  *                             (default 96 MiB; 0 makes every call eligible; negative restores the default)
  *   "region_shift"            a region is 2^value sites (default 23, allowed 4..30; raised automatically so that
  *                             there are at most 32 regions; negative restores the default)
  *   "force_mode"              -1 = the probe decides (default), 0 = always direct, 1 = always bucketed when eligible
- *   "bucket_capacity"         pairs each region's bucket can hold (<= 0: 4 M / regions + 4096); pairs that do not
- *                             fit are joined on the spot by the general algorithm
+ *   "bucket_capacity"         pairs the chunk pool of the bucketed form can hold (<= 0: 1.25 n_bonds + slack); if it
+ *                             runs dry the direct kernel re-does the bond list behind the bucketed kernels
+ *   "scatter_tiles"           1 = the bulk-copy (cp.async.bulk) scatter kernel for 16-byte aligned input (default),
+ *                             0 = the register kernel for everything
+ *   "probe_cache"             1 = remember the probe's answer per bond list (default), 0 = probe on every call
  *   "two_pass"                direct form of step (iii): 0 = one pass over the bonds, 1 = the paper's order of work
  *                             (hook every site to its smallest lower neighbour, flatten, then Algorithm 1; two passes
  *                             over the bonds), -1 = two passes iff n_bonds >= 2.5 n_sites and n_bonds >= 2^20 (default)
- *   "tile_mode"               tiled form of step (iii) for bond lists that are local in the site numbering (window of
- *                             labels in shared memory): 0 = off (default), -1 = a device-side probe
- *                             decides, 1 = always; "sub_shift" (window = 2^value sites, <= 15), "fine_capacity",
- *                             "tile_min_bonds", "small_max_sites" tune it
+ *   "flatten_window_bytes"    step (iv) behind the bucketed form gathers from one window of label[] of this many bytes
+ *                             at a time (default 64 MiB, what stays resident in L2);
+ *   "flatten_window_min_bytes" ... for label arrays of at least this many bytes (default 96 MiB; 0 = always; < 0 = never)
  *   "reset"                   all defaults (value ignored)
  * Unknown names -> CCL_INVALID_ARG. */
 int ccl_set_option(const char* name, int64_t value);
@@ -201,8 +220,9 @@ int ccl_set_option(const char* name, int64_t value);
 /* ---- profiling hook ------------------------------------------------------------------------------------
  *
  * Optional cudaEvent_t handles (as void*, any of them NULL = off) that the NEXT ccl_label / ccl_label_bits calls on
- * this host thread record on their stream: after step (i) (k_init), after step (iii) (k_reduce) and after step
- * (iv) (k_flatten).  Together with an event the caller records before the call they give each step's device time
+ * this host thread record on their stream: after step (i) (k_init; when the bucketed kernels write the labels
+ * region by region themselves there is no separate step (i) and the event falls at the start of step (iii)), after
+ * step (iii) and after step (iv) (k_flatten).  Together with an event the caller records before the call they give each step's device time
  * from inside the caller's own timed region.  The handles stay in force until replaced; pass three NULLs to clear. */
 int ccl_set_profile_events(void* after_init, void* after_reduce, void* after_flatten);
 

@@ -15,8 +15,8 @@ lib = C.CDLL(_LIB_PATH)
 EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangular", "ccl_gen_honeycomb",
            "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
            "ccl_set_profile_events", "ccl_set_option", "ccl_label_batch", "ccl_relabel_sequential", "ccl_gen_cayley3",
-           "ccl_gen_wrap_vectors", "ccl_wrap", "ccl_label_nn", "ccl_label_sweep_host", "ccl_last_error",
-           "ccl_version", "ccl_launch_count"]
+           "ccl_gen_wrap_vectors", "ccl_wrap", "ccl_label_nn", "ccl_label_sweep_host", "ccl_trim_scratch",
+           "ccl_scratch_bytes", "ccl_last_error", "ccl_version", "ccl_launch_count"]
 
 _vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
 lib.ccl_label.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp]
@@ -42,7 +42,9 @@ lib.ccl_gen_wrap_vectors.argtypes = [_i32, _i32, _vp, _vp, _vp]
 lib.ccl_wrap.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
 lib.ccl_label_nn.argtypes = [_i64, _i32, _vp, _vp, _vp]
 lib.ccl_label_sweep_host.argtypes = [_i64, _i64, _vp, _vp, _i32, _vp, _vp, _vp]
-for _n in EXPORTS[:18]:
+lib.ccl_trim_scratch.argtypes = [C.c_size_t, _vp]
+lib.ccl_scratch_bytes.argtypes = [C.POINTER(_i64), C.POINTER(_i64)]
+for _n in EXPORTS[:20]:
     getattr(lib, _n).restype = C.c_int
 
 
@@ -81,10 +83,21 @@ def _dev(t, dtype, what):
     return t.data_ptr()
 
 
+def _sizes(n_sites, n_bonds, labels, mask, mask_len, what):
+    """The C ABI takes bare pointers: refuse tensors that are shorter than the counts say."""
+    if labels.numel() < n_sites:
+        raise ValueError("%s: labels has %d elements, n_sites = %d" % (what, labels.numel(), n_sites))
+    if mask is not None and mask.numel() < mask_len:
+        raise ValueError("%s: the occupancy tensor has %d elements, %d are needed" % (what, mask.numel(), mask_len))
+
+
 def label(n_sites, src, dst, occupied=None, labels=None):
     """ccl_label: uint8 mask (or None = all bonds occupied).  Returns the int32 label tensor."""
     if labels is None:
         labels = torch.empty(n_sites, dtype=torch.int32, device=src.device)
+    if dst.numel() < src.numel():
+        raise ValueError("ccl_label: dst is shorter than src")
+    _sizes(n_sites, src.numel(), labels, occupied, src.numel(), "ccl_label")
     _check(lib.ccl_label(n_sites, src.numel(), _dev(src, torch.int32, "src"), _dev(dst, torch.int32, "dst"),
                          _dev(occupied, torch.uint8, "occupied"), _dev(labels, torch.int32, "labels"), _stream()),
            "ccl_label")
@@ -96,6 +109,9 @@ def label_bits(n_sites, src, dst, occupied_bits, labels=None, n_bonds=None):
     if labels is None:
         labels = torch.empty(n_sites, dtype=torch.int32, device=src.device)
     m = src.numel() if n_bonds is None else n_bonds
+    if src.numel() < m or dst.numel() < m:
+        raise ValueError("ccl_label_bits: src/dst are shorter than n_bonds")
+    _sizes(n_sites, m, labels, occupied_bits, (m + 31) // 32, "ccl_label_bits")
     _check(lib.ccl_label_bits(n_sites, m, _dev(src, torch.int32, "src"), _dev(dst, torch.int32, "dst"),
                               _dev(occupied_bits, torch.int32, "occupied_bits"),
                               _dev(labels, torch.int32, "labels"), _stream()), "ccl_label_bits")
@@ -178,6 +194,18 @@ def set_profile_events(after_init=None, after_reduce=None, after_flatten=None):
 def set_option(name, value=0):
     """ccl_set_option(name, value); see include/ccl.h for the names."""
     _check(lib.ccl_set_option(name.encode(), int(value)), "ccl_set_option")
+
+
+def trim_scratch(keep_bytes=0):
+    """ccl_trim_scratch on torch's current stream (synchronises it)."""
+    _check(lib.ccl_trim_scratch(int(keep_bytes), _stream()), "ccl_trim_scratch")
+
+
+def scratch_bytes():
+    """ccl_scratch_bytes: (reserved, in_use) of the library's memory pool on the current device."""
+    r, u = _i64(0), _i64(0)
+    _check(lib.ccl_scratch_bytes(C.byref(r), C.byref(u)), "ccl_scratch_bytes")
+    return int(r.value), int(u.value)
 
 
 def set_tuning(bucket_min_label_bytes=-1, region_shift=-1, force_mode=-1, bucket_capacity=0):

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libccl.so")
-SOURCES = ["ccl_api.cu", "ccl_label.cu", "ccl_bucket.cu", "ccl_tile.cu", "ccl_batch.cu", "ccl_wrap.cu", "ccl_nn.cu", "ccl_gen.cu", "ccl_stats.cu"]
+SOURCES = ["ccl_api.cu", "ccl_label.cu", "ccl_bucket.cu", "ccl_batch.cu", "ccl_wrap.cu", "ccl_nn.cu", "ccl_gen.cu", "ccl_stats.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
@@ -46,17 +46,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_ubench() -> str:
-    """The random-access microbenchmark of DESIGN.md section 6 (standalone executable, not part of libccl.so)."""
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    out = os.path.join(HERE, "ccl_ubench.bin")
-    subprocess.check_call([nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-o", out,
-                           os.path.join(CSRC, "ccl_ubench.cu")])
-    return out
-
-
 if __name__ == "__main__":
-    if "--ubench" in sys.argv:
-        print(build_ubench())
-    else:
-        print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv))

@@ -2,6 +2,8 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "ccl_common.cuh"
 
 namespace ccl {
@@ -21,17 +23,20 @@ void count_launch(int n) { g_launches += n; }
 
 Tuning& tuning()
 {
-    static Tuning t;
+    static thread_local Tuning t;                  // per host thread, like the error string and the launch counter
     return t;
 }
 
-int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st)
+static std::mutex g_pool_mutex;
+static cudaMemPool_t g_pools[64] = {};
+
+static int pool_for_current_device(cudaMemPool_t* out, bool create)
 {
-    static cudaMemPool_t pools[64] = {};
     int dev = 0;
     CCL_CUDA_TRY(cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64) { set_error("device index %d out of range", dev); return CCL_UNSUPPORTED; }
-    if (pools[dev] == nullptr) {
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (g_pools[dev] == nullptr && create) {
         cudaMemPoolProps props = {};
         props.allocType = cudaMemAllocationTypePinned;
         props.handleTypes = cudaMemHandleTypeNone;
@@ -39,18 +44,27 @@ int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st)
         props.location.id = dev;
         cudaMemPool_t pool = nullptr;
         CCL_CUDA_TRY(cudaMemPoolCreate(&pool, &props));
-        unsigned long long keep = ~0ull;
+        unsigned long long keep = ~0ull;           // freed scratch stays in the pool until ccl_trim_scratch
         CCL_CUDA_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-        pools[dev] = pool;
+        g_pools[dev] = pool;
     }
-    CCL_CUDA_TRY(cudaMallocFromPoolAsync(ptr, bytes, pools[dev], st));
+    *out = g_pools[dev];
+    return CCL_OK;
+}
+
+int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st)
+{
+    cudaMemPool_t pool = nullptr;
+    const int rc = pool_for_current_device(&pool, true);
+    if (rc != CCL_OK) return rc;
+    CCL_CUDA_TRY(cudaMallocFromPoolAsync(ptr, bytes, pool, st));
     return CCL_OK;
 }
 
 }  // namespace ccl
 
 extern "C" const char* ccl_last_error(void) { return ccl::g_error; }
-extern "C" int ccl_version(void) { return 200; }      // 0.2.0: + label_nn, label_batch, label_sweep_host, relabel, wrap
+extern "C" int ccl_version(void) { return 300; }      // 0.3.0: chunked bucket pool, windowed step (iv), scratch trim, per-thread options
 extern "C" int64_t ccl_launch_count(void) { return ccl::g_launches; }
 
 extern "C" int ccl_set_option(const char* name, int64_t value)
@@ -82,25 +96,41 @@ extern "C" int ccl_set_option(const char* name, int64_t value)
     }
     if (!strcmp(name, "bucket_capacity")) { t.bucket_capacity = value > 0 ? value : 0; return CCL_OK; }
     if (!strcmp(name, "two_pass")) { t.two_pass = value > 0 ? 1 : value < 0 ? -1 : 0; return CCL_OK; }
-    if (!strcmp(name, "tile_mode")) {
-        if (value < -1 || value > 1) {
-            ccl::set_error("invalid argument: tile_mode must be -1, 0 or 1");
-            return CCL_INVALID_ARG;
-        }
-        t.tile_mode = (int32_t)value;
+    if (!strcmp(name, "scatter_tiles")) { t.scatter_tiles = value != 0; return CCL_OK; }
+    if (!strcmp(name, "probe_cache")) { t.probe_cache = value != 0; return CCL_OK; }
+    if (!strcmp(name, "flatten_window_bytes")) {
+        t.flatten_window_bytes = value > 0 ? value : def.flatten_window_bytes;
         return CCL_OK;
     }
-    if (!strcmp(name, "sub_shift")) {
-        if (value > 15) {
-            ccl::set_error("invalid argument: sub_shift must be at most 15 (128 KiB of labels in shared memory)");
-            return CCL_INVALID_ARG;
-        }
-        t.sub_shift = value >= 2 ? (int32_t)value : -1;
-        return CCL_OK;
-    }
-    if (!strcmp(name, "fine_capacity")) { t.fine_capacity = value > 0 ? value : 0; return CCL_OK; }
-    if (!strcmp(name, "small_max_sites")) { t.small_max_sites = value >= 0 ? value : def.small_max_sites; return CCL_OK; }
-    if (!strcmp(name, "tile_min_bonds")) { t.tile_min_bonds = value >= 0 ? value : def.tile_min_bonds; return CCL_OK; }
+    if (!strcmp(name, "flatten_window_min_bytes")) { t.flatten_window_min_bytes = value; return CCL_OK; }
     ccl::set_error("invalid argument: unknown option '%s'", name);
     return CCL_INVALID_ARG;
+}
+
+extern "C" int ccl_trim_scratch(size_t keep_bytes, void* stream)
+{
+    using namespace ccl;
+    cudaMemPool_t pool = nullptr;
+    const int rc = pool_for_current_device(&pool, false);
+    if (rc != CCL_OK) return rc;
+    if (pool == nullptr) return CCL_OK;                    // nothing was ever allocated on this device
+    CCL_CUDA_TRY(cudaStreamSynchronize(as_stream(stream)));   // scratch freed on the stream must have been released
+    CCL_CUDA_TRY(cudaMemPoolTrimTo(pool, keep_bytes));
+    return CCL_OK;
+}
+
+extern "C" int ccl_scratch_bytes(int64_t* reserved, int64_t* in_use)
+{
+    using namespace ccl;
+    cudaMemPool_t pool = nullptr;
+    const int rc = pool_for_current_device(&pool, false);
+    if (rc != CCL_OK) return rc;
+    unsigned long long r = 0, u = 0;
+    if (pool != nullptr) {
+        CCL_CUDA_TRY(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReservedMemCurrent, &r));
+        CCL_CUDA_TRY(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrUsedMemCurrent, &u));
+    }
+    if (reserved) *reserved = (int64_t)r;
+    if (in_use) *in_use = (int64_t)u;
+    return CCL_OK;
 }

@@ -1,7 +1,7 @@
 // ccl_bucket.cu -- step (iii) of PAPER.md:113 for label arrays that do not fit in L2: region-bucketed label reduction.
 //
 // Why: on B200 a random atomicMin into a 256 MiB label[] runs at ~31 G/s (every access is an HBM sector fetch plus a
-// write-back), into an L2-resident 32-64 MiB slice at ~130 G/s (profiles/r1_ubench.txt).  So the site range is cut
+// write-back), into an L2-resident 32-64 MiB slice at ~130 G/s (profiles/r1_ubench.md).  So the site range is cut
 // into regions whose labels fit in L2, every occupied bond is filed under the region of its HIGHER endpoint, and the
 // regions are reduced one after the other from the highest down.  Within region r each pair (a, b), a < b, runs
 // Algorithm 1's atomic loop directly on its own endpoints:
@@ -14,10 +14,12 @@
 // The higher site of a pending pair only ever decreases, so a pair either stays in region r (the loop goes on in
 // the same thread) or is re-filed under a LOWER region, which has not been reduced yet.  No root finding and no
 // access outside the region are needed; after region 0 label[] is a forest with label[x] <= x, and step (iv)
-// flattens it.  Measured chain lengths: 1.3-2.2 atomics per occupied bond on random regular graphs.
+// flattens it.  This orders the WORK by region; no region is labeled on its own and nothing is merged across region
+// borders afterwards (reading R14).
 //
-// A device-side probe decides whether to take this form at all: graphs whose bonds are local in the site numbering
-// (raster-ordered lattices) keep the direct one-pass kernel of ccl_label.cu, whose gathers hit L2 anyway.
+// Step (i) rides along: label[] of region r is written (label[i] = i) by the kernel that runs just before
+// k_descend(r), so the lines are still in L2 when the first atomic arrives, and the write to HBM and the fetch back
+// that a separate initialization pass costs disappear.
 #include "ccl_common.cuh"
 #include "ccl_unionfind.cuh"
 #include "ccl_emit.cuh"
@@ -25,20 +27,32 @@
 namespace ccl {
 
 constexpr int kBThreads = 256;
+constexpr int kScatterP = 8;                               // bonds per thread and tile in k_scatter
+constexpr int kDescendP = 4;                               // pairs per thread and tile in k_descend
+
+// label[i] = i for the regions that are touched before any k_descend has run: [lo, n_sites).
+__global__ void __launch_bounds__(kBThreads)
+k_init_top(int64_t lo, int64_t n_sites, int32_t* __restrict__ label)
+{
+    init_range(label, lo, n_sites, (int64_t)blockIdx.x * kBThreads + threadIdx.x, (int64_t)gridDim.x * kBThreads);
+}
 
 // -------------------------------------------------------------------------------------------------- scatter
 // One pass over the bond stream: occupied, non-loop bonds become (lo, hi) pairs filed under region(hi).
+//
+// k_scatter: the general kernel (any alignment, any length), 8 bonds per thread in registers.
 template <int MASK>
 __global__ void __launch_bounds__(kBThreads)
 k_scatter(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-          const void* __restrict__ occ, int vec, int shift, BucketHeader* hdr, int2* buckets,
-          unsigned long long cap, int32_t* label)
+          const void* __restrict__ occ, int vec, BucketRef bk, int gated)
 {
-    constexpr int P = 8;
-    __shared__ EmitSmem<kBThreads, P> sm;
+    constexpr int P = kScatterP;
+    __shared__ EmitSmem sm;
+    __shared__ int2 stage[kBThreads * P];
     pdl_wait();
-    if (hdr->mode != 1) return;
+    if (gated && bk.hdr->mode != 1) return;
     const uint64_t pol = evict_first_policy();
+    emit_begin(sm);
     const int64_t tiles = (n_bonds + kBThreads * P - 1) / (kBThreads * P);
     for (int64_t tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
         const int64_t b0 = (tile * kBThreads + threadIdx.x) * P;
@@ -75,31 +89,178 @@ k_scatter(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __res
             lo[k] = on ? min(u[k], v[k]) : -1;
             hi[k] = max(u[k], v[k]);
         }
-        cta_emit<kBThreads, P>(sm, lo, hi, shift, hdr, buckets, cap, JoinNow{label}, pol);
+        cta_emit<kBThreads, P>(sm, stage, lo, hi, bk, pol);
     }
+    pdl_go();
+}
+
+// k_scatter_tiles: whole tiles of 2048 bonds of 16-byte aligned input.  The kernel above issues ~70 instructions per
+// bond slot and most of them are predicated off (three quarters of the slots hold unoccupied bonds at p = 0.25).  Here a
+// tile -- src, dst and their mask bits -- is copied to shared memory by the bulk-copy engine (cp.async.bulk, completion
+// on an mbarrier; two tiles in flight per CTA, so the HBM stream never waits for the arithmetic); every warp compacts
+// the occupied bonds of its 256 with ballots into an index list and only then forms pairs, with all lanes busy; the
+// pairs are ranked per region, sorted through the staging array (which reuses the tile's own input buffer) and
+// appended to the buckets as in cta_emit.
+constexpr int kTileBonds = 2048;
+template <int MASK>
+struct ScatterTile {
+    int32_t src[kTileBonds];
+    int32_t dst[kTileBonds];               // src + dst are reused as the staging array int2[kTileBonds] of the append
+    uint32_t mask[MASK == 1 ? kTileBonds / 4 : kTileBonds / 32];      // MASK 1: 2048 bytes; MASK 2: 64 words
+};
+template <int MASK>
+struct ScatterSmem {
+    ScatterTile<MASK> in[2];
+    int2 pairs[kTileBonds];                // warp w's compacted pairs at [256 w, 256 w + n_w)
+    uint16_t slot[kTileBonds];             // rank of the pair within its region; the upper half of warp w's 512 bytes
+                                           // first holds the warp's index list (one byte per occupied bond)
+    EmitSmem emit;
+    unsigned long long mbar[2];
+};
+
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void bulk_load(void* dst_smem, const void* src_gmem, uint32_t bytes, unsigned long long* mbar,
+                                          uint64_t pol)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(smem_addr(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_addr(mbar)), "l"(pol)
+                 : "memory");
+}
+
+template <int MASK>
+__device__ __forceinline__ void tile_fetch(ScatterTile<MASK>& t, unsigned long long* mbar, int64_t tile,
+                                           const int32_t* src, const int32_t* dst, const void* occ, uint64_t pol)
+{
+    constexpr uint32_t kMaskBytes = MASK == 2 ? kTileBonds / 8 : MASK == 1 ? kTileBonds : 0;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(mbar)),
+                 "r"((uint32_t)(2 * kTileBonds * sizeof(int32_t)) + kMaskBytes)
+                 : "memory");
+    bulk_load(t.src, src + tile * kTileBonds, kTileBonds * sizeof(int32_t), mbar, pol);
+    bulk_load(t.dst, dst + tile * kTileBonds, kTileBonds * sizeof(int32_t), mbar, pol);
+    if (MASK != 0) bulk_load(t.mask, static_cast<const char*>(occ) + tile * kMaskBytes, kMaskBytes, mbar, pol);
+}
+
+__device__ __forceinline__ void mbar_wait(unsigned long long* mbar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}"
+        ::"r"(smem_addr(mbar)), "r"(parity)
+        : "memory");
+}
+
+template <int MASK>
+__global__ void __launch_bounds__(kBThreads, 4)
+k_scatter_tiles(int64_t n_tiles, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
+                const void* __restrict__ occ, BucketRef bk, int gated)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    ScatterSmem<MASK>& sm = *reinterpret_cast<ScatterSmem<MASK>*>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_addr(&sm.mbar[0])));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_addr(&sm.mbar[1])));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    pdl_wait();
+    if (gated && bk.hdr->mode != 1) return;
+    const uint64_t pol = evict_first_policy();
+    emit_begin(sm.emit);                                   // (barrier: the mbarriers are initialised for everybody)
+    const int64_t stride = gridDim.x;
+    if (tid == 0) {
+        if ((int64_t)blockIdx.x < n_tiles) tile_fetch<MASK>(sm.in[0], &sm.mbar[0], blockIdx.x, src, dst, occ, pol);
+        if ((int64_t)blockIdx.x + stride < n_tiles) tile_fetch<MASK>(sm.in[1], &sm.mbar[1], blockIdx.x + stride, src, dst, occ, pol);
+    }
+    int2* my_pairs = sm.pairs + warp * 256;
+    uint16_t* my_slot = sm.slot + warp * 256;
+    uint8_t* my_idx = reinterpret_cast<uint8_t*>(my_slot) + 256;       // entry j is read before slot j' >= 128 overwrites it
+    int it = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += stride, ++it) {
+        const int cur = it & 1;
+        ScatterTile<MASK>& in = sm.in[cur];
+        mbar_wait(&sm.mbar[cur], (it >> 1) & 1);
+        // ---- the warp's occupied bonds, compacted
+        int n = 0;
+#pragma unroll
+        for (int row = 0; row < 8; ++row) {
+            bool on = true;
+            if (MASK == 2) on = (in.mask[warp * 8 + row] >> lane) & 1u;
+            else if (MASK == 1) on = reinterpret_cast<const uint8_t*>(in.mask)[warp * 256 + row * 32 + lane] != 0;
+            const unsigned bal = __ballot_sync(0xffffffffu, on);
+            if (on) my_idx[n + __popc(bal & ((1u << lane) - 1u))] = (uint8_t)(row * 32 + lane);
+            n += __popc(bal);
+        }
+        __syncwarp();
+        // ---- pairs: (lo, hi) and their rank within the target region
+        for (int j0 = 0; j0 < n; j0 += 32) {
+            const int j = j0 + lane;
+            int32_t lo = -1, hi = 0;
+            if (j < n) {
+                const int b = warp * 256 + my_idx[j];
+                const int32_t u = in.src[b], v = in.dst[b];
+                hi = max(u, v);
+                if (u != v) lo = min(u, v);
+            }
+            __syncwarp();                                  // every lane has read its index byte
+            if (j < n) {
+                my_pairs[j] = make_int2(lo, hi);
+                if (lo >= 0) my_slot[j] = (uint16_t)atomicAdd(&sm.emit.cnt[hi >> bk.shift], 1);
+            }
+        }
+        __syncthreads();                                   // all pairs ranked; nobody reads in.src / in.dst any more
+        int c = 0;
+        unsigned long long base = 0;
+        if (tid < 32) { c = emit_scan(sm.emit); base = emit_reserve(bk, c); }
+        __syncthreads();
+        int2* stage = reinterpret_cast<int2*>(in.src);
+        for (int j = lane; j < n; j += 32) {
+            const int2 pr = my_pairs[j];
+            if (pr.x >= 0) stage[sm.emit.pref[pr.y >> bk.shift] + my_slot[j]] = pr;
+        }
+        if (tid < 32) emit_place(sm.emit, bk, c, base);
+        __syncthreads();
+        emit_copy_out<kBThreads>(sm.emit, stage, bk, pol);
+        __syncthreads();                                   // the buffer is free again
+        if (tid == 0 && tile + 2 * stride < n_tiles) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes (staging) before the bulk copy
+            tile_fetch<MASK>(in, &sm.mbar[cur], tile + 2 * stride, src, dst, occ, pol);
+        }
+    }
+    pdl_go();
 }
 
 // -------------------------------------------------------------------------------------------------- descend
-// Reduce region r: all label[] traffic of this launch falls into [r << shift, (r+1) << shift).
-template <int P>
-__global__ void __launch_bounds__(kBThreads)
-k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long cap, int32_t* label)
+// Reduce region r: all label[] traffic of this launch falls into [r << shift, (r+1) << shift).  init_lo < init_hi: the
+// labels of the region that comes next are written on the way out (step (i) for that region).
+__global__ void __launch_bounds__(kBThreads, 6)
+k_descend(int r, BucketRef bk, int gated, int64_t init_lo, int64_t init_hi, int32_t* label)
 {
-    __shared__ EmitSmem<kBThreads, P> sm;
+    constexpr int P = kDescendP;
+    __shared__ EmitSmem sm;
+    __shared__ int2 stage[kBThreads * P];
     pdl_wait();
-    if (hdr->mode != 1) return;
+    if (gated && bk.hdr->mode != 1) return;
     const uint64_t pol = evict_first_policy();
-    unsigned long long n = hdr->count[r];
-    if (n > cap) n = cap;
-    const int2* bucket = buckets + (size_t)r * cap;
+    const int shift = bk.shift;
+    emit_begin(sm);
+    const unsigned long long n = bk.hdr->count[r];
     const long long tiles = (long long)((n + kBThreads * P - 1) / (kBThreads * P));
     for (long long tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
-        const unsigned long long i0 = ((unsigned long long)tile * kBThreads + threadIdx.x) * P;
+        const unsigned long long t0 = (unsigned long long)tile * kBThreads * P;
+        const int2* base = bucket_tile(bk, r, t0);
+        if (base == nullptr) continue;                                 // dropped (pool dry): CTA-uniform
+        const unsigned long long i0 = t0 + (unsigned long long)threadIdx.x * P;
+        const int2* mine = base + threadIdx.x * P;
         int32_t a[P], b[P], old[P];
         if (i0 + P <= n) {
 #pragma unroll
             for (int q = 0; q < P / 2; ++q) {
-                const int4 v = ld_stream_v4(reinterpret_cast<const int32_t*>(bucket + i0 + 2 * q), pol);
+                const int4 v = ld_stream_v4(reinterpret_cast<const int32_t*>(mine + 2 * q), pol);
                 a[2 * q] = v.x; b[2 * q] = v.y; a[2 * q + 1] = v.z; b[2 * q + 1] = v.w;
             }
         } else {
@@ -107,18 +268,17 @@ k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long
             for (int k = 0; k < P; ++k) {
                 a[k] = -1; b[k] = 0;
                 if (i0 + k < n) {
-                    a[k] = ld_stream_s32(reinterpret_cast<const int32_t*>(bucket + i0 + k), pol);
-                    b[k] = ld_stream_s32(reinterpret_cast<const int32_t*>(bucket + i0 + k) + 1, pol);
+                    a[k] = ld_stream_s32(reinterpret_cast<const int32_t*>(mine + k), pol);
+                    b[k] = ld_stream_s32(reinterpret_cast<const int32_t*>(mine + k) + 1, pol);
                 }
             }
         }
-        // first atomics of the four pairs in flight together
+        // first atomics of the P pairs in flight together
 #pragma unroll
         for (int k = 0; k < P; ++k) old[k] = (a[k] >= 0) ? atomicMin(label + b[k], a[k]) : a[k];
         // Continuation: the pairs whose first atomic found b linked already.  The P chains of a thread advance together,
         // one link per round with their loads (and then their atomics) in flight at the same time; walked one after the
-        // other they made the last region, where every chain of the giant cluster ends, pure memory latency (0.42 ms
-        // at p = 0.45 on config 5).
+        // other they made the last region, where every chain of the giant cluster ends, pure memory latency.
         bool act[P], pend[P];
 #pragma unroll
         for (int k = 0; k < P; ++k) { act[k] = a[k] >= 0 && old[k] != b[k] && old[k] != a[k]; pend[k] = false; }
@@ -147,63 +307,135 @@ k_descend(int r, int shift, BucketHeader* hdr, int2* buckets, unsigned long long
                 if (act[k]) { act[k] = old[k] != b[k] && old[k] != a[k]; any |= act[k]; }
             if (!any) break;
         }
+        bool pending = false;
 #pragma unroll
-        for (int k = 0; k < P; ++k) if (!pend[k]) a[k] = -1;
-        cta_emit<kBThreads, P>(sm, a, b, shift, hdr, buckets, cap, JoinNow{label}, pol);
+        for (int k = 0; k < P; ++k) { if (!pend[k]) a[k] = -1; pending |= pend[k]; }
+        if (__syncthreads_or(pending)) cta_emit<kBThreads, P>(sm, stage, a, b, bk, pol);
     }
+    if (init_lo < init_hi)
+        init_range(label, init_lo, init_hi, (int64_t)blockIdx.x * kBThreads + threadIdx.x, (int64_t)gridDim.x * kBThreads);
     pdl_go();                                              // this CTA is done: the next launch may take its place
 }
 
 // ------------------------------------------------------------------------------------------------- host side
-int bucketed_begin(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, cudaStream_t st,
-                   BucketPlan* plan, ProbeJob* job, void** ws_out)
+// Persistent grids: as many CTAs as are resident at once (every CTA works through the same number of tiles, so a CTA
+// that had to wait for a free slot would finish alone).
+template <typename K>
+static int resident_grid(K kernel, size_t smem)
+{
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kBThreads, smem) != cudaSuccess) per_sm = 0;
+    cudaGetLastError();
+    if (per_sm < 1) per_sm = 1;
+    int sms = kSMs, dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    return per_sm * (sms > 0 ? sms : kSMs);
+}
+
+struct BucketGrids { int scatter = 0, tiles[3] = {0, 0, 0}, descend = 0; };
+static const BucketGrids& bucket_grids()
+{
+    static BucketGrids g;
+    if (g.descend == 0) {
+        g.scatter = resident_grid(k_scatter<2>, 0);
+        cudaFuncSetAttribute(k_scatter_tiles<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem<0>));
+        cudaFuncSetAttribute(k_scatter_tiles<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem<1>));
+        cudaFuncSetAttribute(k_scatter_tiles<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem<2>));
+        g.tiles[0] = resident_grid(k_scatter_tiles<0>, sizeof(ScatterSmem<0>));
+        g.tiles[1] = resident_grid(k_scatter_tiles<1>, sizeof(ScatterSmem<1>));
+        g.tiles[2] = resident_grid(k_scatter_tiles<2>, sizeof(ScatterSmem<2>));
+        g.descend = resident_grid(k_descend, 0);
+    }
+    return g;
+}
+
+int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, cudaStream_t st, BucketPlan* plan, void** ws_out)
 {
     // region size: 2^23 sites (32 MiB of labels) unless that would need more than kMaxRegions regions
-    int shift = tuning().region_shift;
+    int shift = t.region_shift;
     while (((n_sites - 1) >> shift) + 1 > kMaxRegions) ++shift;
     const int n_regions = (int)(((n_sites - 1) >> shift) + 1);
-    unsigned long long cap = (unsigned long long)((4 * n_bonds) / n_regions + 4096);
-    if (tuning().bucket_capacity > 0) cap = (unsigned long long)tuning().bucket_capacity;
-    cap = (cap + 7ull) & ~7ull;                                   // keeps every bucket 64-byte aligned
+    // Pool: room for 1.25 pairs per bond (every occupied bond, and what the descent re-files) in chunks of about 1/64 of
+    // that, plus the chunk every region leaves partly filled.
+    int cshift = kMinChunkShift;
+    while (cshift < kMaxChunkShift && (n_bonds >> (cshift + 6)) > 0) ++cshift;
+    unsigned long long n_chunks;
+    if (t.bucket_capacity > 0) n_chunks = (((unsigned long long)t.bucket_capacity - 1) >> cshift) + 1;
+    else n_chunks = (((unsigned long long)n_bonds * 5 / 4) >> cshift) + (unsigned long long)n_regions + 2;
+    if (n_chunks > 0x7FFFFFF0ull) n_chunks = 0x7FFFFFF0ull;
     const size_t hdr_bytes = (sizeof(BucketHeader) + 255) & ~(size_t)255;
-    const size_t bytes = hdr_bytes + (size_t)n_regions * cap * sizeof(int2);
+    const size_t table_bytes = (((size_t)n_regions * n_chunks * sizeof(unsigned int)) + 255) & ~(size_t)255;
+    const size_t bytes = hdr_bytes + table_bytes + ((size_t)n_chunks << cshift) * sizeof(int2);
     void* ws = nullptr;
     { const int rc = scratch_alloc(&ws, bytes, st); if (rc != CCL_OK) return rc; }
     *ws_out = ws;
     plan->hdr = static_cast<BucketHeader*>(ws);
-    plan->buckets = static_cast<char*>(ws) + hdr_bytes;
-    plan->cap = cap;
+    plan->table = reinterpret_cast<unsigned int*>(static_cast<char*>(ws) + hdr_bytes);
+    plan->pool = reinterpret_cast<int2*>(static_cast<char*>(ws) + hdr_bytes + table_bytes);
+    plan->n_chunks = (unsigned int)n_chunks;
+    plan->stride = (unsigned int)n_chunks;
     plan->shift = shift;
+    plan->cshift = cshift;
     plan->n_regions = n_regions;
-    job->hdr = plan->hdr;
-    job->n_bonds = n_bonds;
-    job->src = src;
-    job->dst = dst;
-    job->shift = shift;
-    job->force_mode = tuning().force_mode;
-    CCL_CUDA_TRY(cudaMemsetAsync(plan->hdr, 0, sizeof(BucketHeader), st));
+    plan->scatter_tiles = t.scatter_tiles;
+    CCL_CUDA_TRY(cudaMemsetAsync(ws, 0, hdr_bytes + table_bytes, st));
     return CCL_OK;
 }
 
-int bucketed_launch(const BucketPlan& plan, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                    int mask_kind, int32_t* labels, cudaStream_t st)
+int bucketed_launch(const BucketPlan& plan, int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+                    const void* occ, int mask_kind, int32_t* labels, cudaStream_t st)
 {
-    BucketHeader* hdr = plan.hdr;
-    int2* buckets = static_cast<int2*>(plan.buckets);
-    const unsigned long long cap = plan.cap;
-    const int shift = plan.shift;
+    BucketRef bk;
+    bk.hdr = plan.hdr; bk.table = plan.table; bk.pool = plan.pool;
+    bk.n_chunks = plan.n_chunks; bk.stride = plan.stride; bk.shift = plan.shift; bk.cshift = plan.cshift;
+    const int R = plan.n_regions, shift = plan.shift;
     const uintptr_t al = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     const int vec = (al & 15) == 0;
-    const int grid = kSMs * 6;
-    if (occ == nullptr)
-        CCL_CUDA_TRY(launch_pdl(k_scatter<0>, (unsigned)grid, (unsigned)kBThreads, st, n_bonds, src, dst, (const void*)nullptr, vec, shift, hdr, buckets, cap, labels));
-    else if (mask_kind == 1)
-        CCL_CUDA_TRY(launch_pdl(k_scatter<1>, (unsigned)grid, (unsigned)kBThreads, st, n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels));
-    else
-        CCL_CUDA_TRY(launch_pdl(k_scatter<2>, (unsigned)grid, (unsigned)kBThreads, st, n_bonds, src, dst, occ, vec, shift, hdr, buckets, cap, labels));
-    count_launch();
-    for (int r = plan.n_regions - 1; r >= 0; --r) {
-        CCL_CUDA_TRY(launch_pdl(k_descend<4>, (unsigned)grid, (unsigned)kBThreads, st, r, shift, hdr, buckets, cap, labels));
+    const BucketGrids& grids = bucket_grids();
+    const int mk = occ == nullptr ? 0 : mask_kind;
+    // the top region must hold label[i] = i before the first k_descend touches it; every k_descend writes the labels
+    // of the region that comes next
+    if (plan.lazy_init) {
+        const int64_t lo = (int64_t)(R - 1) << shift;
+        int64_t blocks = ((n_sites - lo + 3) / 4 + kBThreads - 1) / kBThreads;
+        if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+        k_init_top<<<(unsigned)blocks, kBThreads, 0, st>>>(lo, n_sites, labels);
+        CCL_CHECK_LAUNCH("k_init_top");
+    }
+    const int gated = plan.gated;
+    // whole tiles of 16-byte aligned input go through the bulk-copy kernel, the rest (a tail, or everything) through
+    // the register kernel
+    int64_t done = 0;
+    const bool mask_ok = occ == nullptr || (reinterpret_cast<uintptr_t>(occ) & 15) == 0;
+    if (vec && mask_ok && plan.scatter_tiles && n_bonds >= kTileBonds) {
+        const int64_t n_tiles = n_bonds / kTileBonds;
+        int tg = grids.tiles[mk];
+        if (tg > n_tiles) tg = (int)n_tiles;
+        if (mk == 0) CCL_CUDA_TRY(launch_pdl_smem(k_scatter_tiles<0>, (unsigned)tg, (unsigned)kBThreads, sizeof(ScatterSmem<0>), st, n_tiles, src, dst, (const void*)nullptr, bk, gated));
+        else if (mk == 1) CCL_CUDA_TRY(launch_pdl_smem(k_scatter_tiles<1>, (unsigned)tg, (unsigned)kBThreads, sizeof(ScatterSmem<1>), st, n_tiles, src, dst, occ, bk, gated));
+        else CCL_CUDA_TRY(launch_pdl_smem(k_scatter_tiles<2>, (unsigned)tg, (unsigned)kBThreads, sizeof(ScatterSmem<2>), st, n_tiles, src, dst, occ, bk, gated));
+        count_launch();
+        done = n_tiles * kTileBonds;
+    }
+    if (done < n_bonds) {
+        const int64_t rest = n_bonds - done;
+        const int32_t *s2 = src + done, *d2 = dst + done;
+        const int vec2 = ((reinterpret_cast<uintptr_t>(s2) | reinterpret_cast<uintptr_t>(d2)) & 15) == 0;
+        const unsigned sg = (unsigned)grids.scatter;
+        if (mk == 0) CCL_CUDA_TRY(launch_pdl(k_scatter<0>, sg, (unsigned)kBThreads, st, rest, s2, d2, (const void*)nullptr, vec2, bk, gated));
+        else if (mk == 1) CCL_CUDA_TRY(launch_pdl(k_scatter<1>, sg, (unsigned)kBThreads, st, rest, s2, d2, (const void*)(static_cast<const uint8_t*>(occ) + done), vec2, bk, gated));
+        else CCL_CUDA_TRY(launch_pdl(k_scatter<2>, sg, (unsigned)kBThreads, st, rest, s2, d2, (const void*)(static_cast<const uint32_t*>(occ) + done / 32), vec2, bk, gated));
+        count_launch();
+    }
+    for (int r = R - 1; r >= 0; --r) {
+        // the kernel before k_descend(r - 1) writes that region's labels, unless they were written up front
+        int64_t init_lo = 0, init_hi = 0;
+        if (plan.lazy_init && r >= 1) {
+            init_lo = (int64_t)(r - 1) << shift;
+            init_hi = (int64_t)r << shift;
+            if (init_hi > n_sites) init_hi = n_sites;
+        }
+        CCL_CUDA_TRY(launch_pdl(k_descend, (unsigned)grids.descend, (unsigned)kBThreads, st, r, bk, gated, init_lo, init_hi, labels));
         count_launch();
     }
     return CCL_OK;

@@ -72,83 +72,77 @@ inline cudaError_t launch_pdl(void (*kernel)(Params...), unsigned grid, unsigned
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
 }
 
+template <typename... Params, typename... Args>
+inline cudaError_t launch_pdl_smem(void (*kernel)(Params...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
+}
+
 // ---- region-bucketed label reduction (ccl_bucket.cu) -----------------------------------------------------
 constexpr int kMaxRegions = 32;
+constexpr int kMinChunkShift = 11, kMaxChunkShift = 21;   // a bucket is a sequence of chunks of 2^11 .. 2^21 pairs
 
 struct BucketHeader {                              // lives in device memory at the head of the call's workspace
-    int32_t mode;                                  // written by probe_regions: 0 = direct kernel, 1 = bucketed, 2 = nothing
-    int32_t pad;
-    unsigned long long count[kMaxRegions];         // pairs filed under each region (may exceed the capacity: the
-                                                   // excess was joined on the spot by the general algorithm)
+    int32_t mode;                                  // written by probe_regions: 0 = direct kernels, 1 = bucketed kernels
+    int32_t overflow;                              // != 0: the chunk pool ran dry and pairs were dropped; the direct kernel
+                                                   // then runs over the whole bond list behind the bucketed kernels
+    unsigned int next_chunk;                       // chunks handed out so far
+    unsigned int pad;
+    unsigned long long count[kMaxRegions];         // pairs filed under each region (logical length of its bucket)
 };
 
-// Header of the tiled form's workspace (ccl_tile.cu).  Starts with a BucketHeader so that k_descend and cta_emit work
-// on the region buckets unchanged.
-constexpr int kMaxSubRegions = 2048;               // sub-regions (tiles of label[] held in shared memory) per call
-constexpr int kFineStride = 8;                     // one fine counter per 32-byte sector (no false sharing in L2)
-struct TileHeader {
-    BucketHeader bh;
-    unsigned long long overflow;                   // pairs in the overflow list
-    unsigned long long pad;
-    unsigned int fine[kMaxSubRegions * kFineStride];   // pairs filed under sub-region s: fine[s * kFineStride]
-};
-
-struct Tuning {                                    // ccl_set_option(); process-wide
+struct Tuning {                                    // ccl_set_option(); one set of knobs per host thread
     int64_t bucket_min_label_bytes = 96ll << 20;   // label[] beyond this cannot stay resident in the 126 MB L2
     int64_t bucket_min_bonds = 1 << 20;
     int32_t region_shift = 23;                     // 2^23 sites = 32 MiB of labels per region
     int32_t force_mode = -1;                       // -1: device-side probe decides; 0: direct; 1: bucketed
-    int64_t bucket_capacity = 0;                   // pairs per region bucket; 0 = 4 M / regions + 4096
+    int64_t bucket_capacity = 0;                   // pairs the chunk pool can hold; 0 = 5 M / 4 + slack
     int32_t two_pass = -1;                         // direct form of step (iii): 0 one pass (k_reduce), 1 hook + flatten +
                                                    // join (the paper's order), -1 by bonds per site (>= 2.5: two passes)
-    int32_t tile_mode = 0;                         // tiled form (ccl_tile.cu): 0 off (default: measured slower, see
-                                                   // profiles/r1_notes.md), -1 a device-side probe decides, 1 always
-    int32_t sub_shift = -1;                        // 2^sub_shift sites per sub-region; -1 = from n_sites
-    int64_t fine_capacity = 0;                     // pairs per sub-region bucket; 0 = 2 M / S + 8192
-    int64_t tile_min_bonds = 1 << 18;
-    int64_t small_max_sites = 1 << 15;             // one-CTA kernel for label arrays up to this many sites              // auto: calls with fewer bonds keep the direct kernel
+    int32_t scatter_tiles = 1;                     // 1: k_scatter_tiles (bulk copies into shared memory) for aligned input
+    int32_t probe_cache = 1;                       // remember the probe's answer per bond list (host side, hint only)
+    int64_t flatten_window_bytes = 64ll << 20;     // step (iv) gathers from one L2-resident window of label[] at a time
+    int64_t flatten_window_min_bytes = 96ll << 20; // ... for label arrays of at least this size (0: always; < 0: never)
 };
 Tuning& tuning();
 
-// The library's own stream-ordered memory pool on the current device (created on first use, release threshold
-// unlimited, so scratch freed by one call is reused by the next instead of going back to the driver).
+// The library's own stream-ordered memory pool on the current device (created on first use; ccl_trim_scratch returns
+// what it holds to the driver), so scratch freed by one call is reused by the next.
 int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st);
 
-// Enqueues probe + scatter + one descend launch per region.  *ws_out is a cudaMallocAsync allocation the caller
-// frees (cudaFreeAsync) after the kernels that read *hdr_out have been enqueued.
-// The region-bucketed form in two halves, so that its probe can ride in k_init (one block of k_init samples the bond
-// list while the others write label[i] = i; as a kernel of its own the probe was 12 us of pure latency on the critical
-// path of every call).  bucketed_begin allocates and clears the workspace and fills in the probe job;
-// bucketed_launch enqueues the scatter and one descend launch per region.  *ws_out is a cudaMallocAsync allocation the
-// caller frees (cudaFreeAsync) after the kernels that read the header have been enqueued.
-struct ProbeJob {
+struct ProbeJob {                                  // the region probe rides in block 0 of k_init (ccl_label.cu)
     BucketHeader* hdr = nullptr;                   // NULL: no probe
     int64_t n_bonds = 0;
     const int32_t* src = nullptr;
     const int32_t* dst = nullptr;
     int shift = 0;
-    int force_mode = -1;
 };
 struct BucketPlan {
     BucketHeader* hdr = nullptr;
-    void* buckets = nullptr;
-    unsigned long long cap = 0;
+    unsigned int* table = nullptr;                 // table[r * stride + k] = 1 + pool index of the k-th chunk of bucket r
+    int2* pool = nullptr;
+    unsigned int n_chunks = 0, stride = 0;
     int shift = 0, n_regions = 0;
+    int cshift = kMinChunkShift;                   // chunk = 2^cshift pairs
+    int scatter_tiles = 1;
+    int lazy_init = 0;                             // 1: label[] of region r is written by the kernel that runs before k_descend(r)
+    int gated = 0;                                 // 1: the kernels return at once unless hdr->mode == 1 (probe undecided on the host)
 };
-int bucketed_begin(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, cudaStream_t st,
-                   BucketPlan* plan, ProbeJob* job, void** ws_out);
-int bucketed_launch(const BucketPlan& plan, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                    int mask_kind, int32_t* labels, cudaStream_t st);
-
-// Tiled form of steps (i)-(iii) for bond lists that are local in the site numbering (ccl_tile.cu).  *done says what
-// was enqueued: kTiledNo nothing (call outside its range); kTiledFinal labels are final (one-CTA kernel); kTiledIfLocal
-// a device-side probe decides -- *not_local points at a device flag that is 0 if the tiled kernels did steps (i)-(iii)
-// and non-zero if they returned at once, so the caller enqueues the other forms gated on it; kTiledForced the tiled
-// kernels ran unconditionally.  *ws_out (if set) is freed by the caller with cudaFreeAsync after the last kernel that
-// reads the flag has been enqueued.
-enum { kTiledNo = 0, kTiledFinal = 1, kTiledIfLocal = 2, kTiledForced = 3 };
-int tiled_reduce(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                 int mask_kind, int32_t* labels, cudaStream_t st, int* done, const int32_t** not_local, void** ws_out);
+// bucketed_begin allocates and clears the workspace (*ws_out: the caller frees it with cudaFreeAsync after the last
+// kernel that reads it has been enqueued); bucketed_launch enqueues k_scatter and one k_descend per region.
+int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, cudaStream_t st, BucketPlan* plan, void** ws_out);
+int bucketed_launch(const BucketPlan& plan, int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
+                    const void* occ, int mask_kind, int32_t* labels, cudaStream_t st);
 
 // ---- device helpers --------------------------------------------------------------------------------------
 // Streaming (read-once) loads: bypass L1 allocation and mark the L2 line evict-first, so that the bond stream
@@ -193,12 +187,11 @@ __device__ __forceinline__ void st_stream_pair(int2* p, int2 v, uint64_t pol)
 }
 
 // Samples up to 8192 bonds at a fixed stride and looks at how many join two different regions (random numbering: 1 - 1/R of
-// them; raster-ordered lattice: only those on region borders): mode 1 = region-bucketed form, 0 = direct kernel.  Called
-// by all threads of ONE block; gated = another form has done the work (mode 2: nothing to do).
-__device__ __forceinline__ void probe_regions(const ProbeJob& job, bool gated)
+// them; raster-ordered lattice: only those on region borders): mode 1 = region-bucketed form, 0 = direct kernels.  Called
+// by all threads of ONE block.
+__device__ __forceinline__ void probe_regions(const ProbeJob& job)
 {
     __shared__ int s_cross;
-    if (gated) { if (threadIdx.x == 0) job.hdr->mode = 2; return; }
     if (threadIdx.x == 0) s_cross = 0;
     __syncthreads();
     const int64_t samples = job.n_bonds < 8192 ? job.n_bonds : 8192;
@@ -212,8 +205,7 @@ __device__ __forceinline__ void probe_regions(const ProbeJob& job, bool gated)
     for (int o = 16; o > 0; o >>= 1) cross += __shfl_xor_sync(0xffffffffu, cross, o);
     if ((threadIdx.x & 31) == 0 && cross) atomicAdd(&s_cross, cross);
     __syncthreads();
-    if (threadIdx.x == 0)
-        job.hdr->mode = job.force_mode >= 0 ? job.force_mode : ((4 * (int64_t)s_cross >= samples) ? 1 : 0);
+    if (threadIdx.x == 0) job.hdr->mode = (4 * (int64_t)s_cross >= samples) ? 1 : 0;
 }
 
 // Label reads during root finding and flattening go through L1 (ld.global.ca).  L1 is not coherent, so a read may
@@ -231,6 +223,46 @@ __device__ __forceinline__ int32_t ld_label(const int32_t* p)
 __device__ __forceinline__ void st_label(int32_t* p, int32_t v)
 {
     asm volatile("st.relaxed.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// read-once load of data this thread may write afterwards (no .nc): skips L1 allocation, evict-first in L2
+__device__ __forceinline__ int4 ld_once_v4(const int32_t* p, uint64_t pol)
+{
+    int4 r;
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.s32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p), "l"(pol)
+                 : "memory");
+    return r;
+}
+__device__ __forceinline__ void st_stream_v4(int32_t* p, int4 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v4.s32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+                 "r"(v.w), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p)
+{
+    unsigned int r;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(r) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v)
+{
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// label[i] = i for i in [lo, hi), lo a multiple of 4, 16-byte stores; called by `nthreads` threads with ranks `rank`.
+__device__ __forceinline__ void init_range(int32_t* __restrict__ label, int64_t lo, int64_t hi, int64_t rank, int64_t nthreads)
+{
+    for (int64_t i = lo + rank * 4; i < hi; i += nthreads * 4) {
+        if (i + 4 <= hi) {
+            const int32_t b = (int32_t)i;
+            *reinterpret_cast<int4*>(label + i) = make_int4(b, b + 1, b + 2, b + 3);   // label is 16 B aligned
+        } else {
+            for (int64_t j = i; j < hi; ++j) label[j] = (int32_t)j;
+        }
+    }
 }
 
 }  // namespace ccl

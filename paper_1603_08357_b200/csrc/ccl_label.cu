@@ -18,21 +18,22 @@ constexpr int kThreads = 256;
 
 // ------------------------------------------------------------------------------------------------ step (i)
 __global__ void __launch_bounds__(kThreads)
-k_init(int64_t n_sites, int32_t* __restrict__ label, const int32_t* gate, ProbeJob job)
+k_init(int64_t n_sites, int32_t* __restrict__ label, ProbeJob job)
 {
-    const bool gated = gate != nullptr && *gate == 0;      // the tiled form (ccl_tile.cu) has written every label
     // the probe of the region-bucketed form rides along in block 0, which starts first (ccl_common.cuh)
-    if (job.hdr != nullptr && blockIdx.x == 0) probe_regions(job, gated);
-    if (gated) return;
-    const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
-    for (int64_t i = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; i < n_sites; i += stride) {
-        if (i + 4 <= n_sites) {
-            const int32_t b = (int32_t)i;
-            *reinterpret_cast<int4*>(label + i) = make_int4(b, b + 1, b + 2, b + 3);   // label is 16 B aligned
-        } else {
-            for (int64_t j = i; j < n_sites; ++j) label[j] = (int32_t)j;
-        }
-    }
+    if (job.hdr != nullptr && blockIdx.x == 0) probe_regions(job);
+    init_range(label, 0, n_sites, (int64_t)blockIdx.x * kThreads + threadIdx.x, (int64_t)gridDim.x * kThreads);
+}
+
+// Which of the enqueued forms of step (iii) runs is decided on the device when the host does not know yet whether the
+// bond list is local in the site numbering (BucketHeader::mode, written by the probe) -- no host round trip.
+enum { kGateNone = 0, kGateDirect = 1, kGateDirectOrOverflow = 2, kGateOverflow = 3 };
+__device__ __forceinline__ bool gate_open(const BucketHeader* hdr, int kind)
+{
+    if (kind == kGateNone) return true;
+    if (kind == kGateDirect) return hdr->mode == 0;
+    if (kind == kGateDirectOrOverflow) return hdr->mode == 0 || hdr->overflow != 0;
+    return hdr->overflow != 0;
 }
 
 // ---------------------------------------------------------------------------------------------- step (iii)
@@ -111,12 +112,11 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
 template <int MASK, bool VEC>
 __global__ void __launch_bounds__(kThreads)
 k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
+         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, int gate)
 {
     __shared__ int2 queue[kThreads / 32][128];
     pdl_wait();
-    if (hdr != nullptr && hdr->mode != 0) return;          // the bucketed form (ccl_bucket.cu) did step (iii)
-    if (gate != nullptr && *gate == 0) return;             // the tiled form (ccl_tile.cu) did
+    if (!gate_open(hdr, gate)) return;                     // the bucketed form (ccl_bucket.cu) did step (iii)
     const uint64_t pol = evict_first_policy();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
@@ -154,10 +154,10 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
 template <int MASK>
 __global__ void __launch_bounds__(kThreads)
 k_hook(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, const void* __restrict__ occ,
-       int vec, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
+       int vec, int32_t* label, const BucketHeader* hdr, int gate)
 {
     pdl_wait();
-    if ((hdr != nullptr && hdr->mode != 0) || (gate != nullptr && *gate == 0)) return;      // another form did step (iii)
+    if (!gate_open(hdr, gate)) return;                     // another form did step (iii)
     const uint64_t pol = evict_first_policy();
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
     for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_bonds; b0 += stride) {
@@ -171,11 +171,11 @@ k_hook(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restri
 template <int MASK>
 __global__ void __launch_bounds__(kThreads)
 k_join(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, const void* __restrict__ occ,
-       int vec, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
+       int vec, int32_t* label, const BucketHeader* hdr, int gate)
 {
     __shared__ int2 queue[kThreads / 32][128];
     pdl_wait();
-    if ((hdr != nullptr && hdr->mode != 0) || (gate != nullptr && *gate == 0)) return;
+    if (!gate_open(hdr, gate)) return;
     const uint64_t pol = evict_first_policy();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
@@ -218,43 +218,88 @@ k_join(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restri
 // Every site follows its chain to the root and stores it (reading R2: per-site chase).  Concurrent
 // writers only ever replace a chain pointer by the root of the same chain, so a reader sees either and still
 // arrives at the root.  Roots and already-flat sites are not rewritten.
+//
+// One launch covers the sites [lo, n_sites) and resolves those whose label lies in the window [lo, hi).  With
+// (lo, hi) = (0, n_sites) that is the whole analysis step.  For label arrays beyond L2 the windows are taken in
+// ascending order, one launch each: label[x] <= x always, so when the window [lo, hi) runs every label below lo is
+// final (a root) -- a chase that starts in the window either ends at a root inside it or leaves it downwards and is
+// then finished.  All gathers of one launch fall into the window, which stays L2-resident, while the sites above it
+// stream past once (evict-first).  A random gather into 256 MiB costs an HBM sector fetch each; into 64 MiB it is an
+// L2 hit.
 __global__ void __launch_bounds__(kThreads)
-k_flatten(int64_t n_sites, int32_t* label, const BucketHeader* hdr, const int32_t* gate)
+k_flatten(int64_t n_sites, int32_t* label, int64_t lo, int64_t hi, const BucketHeader* hdr, int gate)
 {
     pdl_wait();
-    if ((hdr != nullptr && hdr->mode != 0) || (gate != nullptr && *gate == 0)) return;      // only for the mid-call flatten
-    const int64_t i0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
-    if (i0 >= n_sites) return;
-    if (i0 + 4 <= n_sites) {
-        int4 l = *reinterpret_cast<const int4*>(label + i0);
-        int32_t cur[4] = {l.x, l.y, l.z, l.w};
-        int32_t par[4];
+    if (!gate_open(hdr, gate)) return;                     // only for the mid-call flatten of the two-pass form
+    constexpr int S = 4, G = 1;                            // four sites (one 16-byte group) per thread
+    // the groups of a thread lie kThreads groups apart, so that a warp's loads stay contiguous
+    const int64_t g0 = lo + ((int64_t)blockIdx.x * kThreads * G + threadIdx.x) * 4;
+    const int32_t wlo = (int32_t)lo, whi = (int32_t)(hi - 1);          // window = [wlo, whi]
+    const uint64_t pol = evict_first_policy();
+    int32_t cur[S], c[S], par[S];
+    bool w[S], full[G], above[G], any = false;
 #pragma unroll
-        for (int k = 0; k < 4; ++k) par[k] = (cur[k] == (int32_t)(i0 + k)) ? cur[k] : ld_label(label + cur[k]);
-        // the four chases advance together: one round = up to four independent loads in flight
-        int32_t c[4] = {cur[0], cur[1], cur[2], cur[3]};
-        for (;;) {
-            bool w[4], any = false;
+    for (int g = 0; g < G; ++g) {
+        const int64_t i0 = g0 + (int64_t)g * kThreads * 4;
+        full[g] = i0 + 4 <= n_sites;
+        above[g] = i0 >= hi;                                           // streams past: read once, written at most once
+        int4 l = make_int4(0, 0, 0, 0);
+        if (full[g]) l = above[g] ? ld_once_v4(label + i0, pol) : *reinterpret_cast<const int4*>(label + i0);
+        cur[4 * g] = l.x; cur[4 * g + 1] = l.y; cur[4 * g + 2] = l.z; cur[4 * g + 3] = l.w;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) { w[k] = par[k] != c[k]; any |= w[k]; }
-            if (!any) break;
-#pragma unroll
-            for (int k = 0; k < 4; ++k) if (w[k]) c[k] = par[k];
-            int32_t nx[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) nx[k] = w[k] ? ld_label(label + c[k]) : par[k];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) par[k] = nx[k];
-        }
-        const bool changed = (c[0] != cur[0]) | (c[1] != cur[1]) | (c[2] != cur[2]) | (c[3] != cur[3]);
-        if (changed) *reinterpret_cast<int4*>(label + i0) = make_int4(c[0], c[1], c[2], c[3]);
-    } else {
-        for (int64_t i = i0; i < n_sites; ++i) {
-            int32_t c = label[i], p = ld_label(label + c);
-            while (p != c) { c = p; p = ld_label(label + c); }
-            label[i] = c;
+        for (int k = 0; k < 4; ++k) {
+            const int q = 4 * g + k;
+            c[q] = cur[q];
+            w[q] = full[g] && cur[q] != (int32_t)(i0 + k) && cur[q] >= wlo && cur[q] <= whi;
+            any |= w[q];
         }
     }
+    if (any) {
+        // the chases advance together: one round = up to S independent loads in flight
+#pragma unroll
+        for (int q = 0; q < S; ++q) par[q] = w[q] ? ld_label(label + c[q]) : c[q];
+        for (;;) {
+            any = false;
+#pragma unroll
+            for (int q = 0; q < S; ++q) {
+                if (w[q]) {
+                    if (par[q] == c[q]) w[q] = false;                               // c is a root
+                    else if (par[q] < wlo) { c[q] = par[q]; w[q] = false; }          // left the window: final
+                    else c[q] = par[q];
+                }
+                any |= w[q];
+            }
+            if (!any) break;
+#pragma unroll
+            for (int q = 0; q < S; ++q) if (w[q]) par[q] = ld_label(label + c[q]);
+        }
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const int64_t i0 = g0 + (int64_t)g * kThreads * 4;
+            const bool changed = (c[4 * g] != cur[4 * g]) | (c[4 * g + 1] != cur[4 * g + 1]) | (c[4 * g + 2] != cur[4 * g + 2]) |
+                                 (c[4 * g + 3] != cur[4 * g + 3]);
+            if (changed) {
+                const int4 out = make_int4(c[4 * g], c[4 * g + 1], c[4 * g + 2], c[4 * g + 3]);
+                if (above[g]) st_stream_v4(label + i0, out, pol);
+                else *reinterpret_cast<int4*>(label + i0) = out;
+            }
+        }
+    }
+    // the ragged end of the array (fewer than four sites), by the thread whose group it would have been
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        const int64_t i0 = g0 + (int64_t)g * kThreads * 4;
+        if (!full[g] && i0 < n_sites) {
+            for (int64_t i = i0; i < n_sites; ++i) {
+                int32_t x = label[i];
+                if (x == (int32_t)i || x < wlo || x > whi) continue;
+                int32_t p = ld_label(label + x);
+                while (p != x && p >= wlo) { x = p; p = ld_label(label + x); }
+                label[i] = (p == x) ? x : p;
+            }
+        }
+    }
+    pdl_go();
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -286,7 +331,7 @@ static int check_args(int64_t n_sites, int64_t n_bonds, const void* src, const v
 
 template <int MASK>
 static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                         int32_t* labels, const BucketHeader* hdr, const int32_t* gate, cudaStream_t st)
+                         int32_t* labels, const BucketHeader* hdr, int gate, cudaStream_t st)
 {
     const int64_t groups = (n_bonds + 3) / 4;
     int64_t blocks = (groups + kThreads - 1) / kThreads;
@@ -294,19 +339,25 @@ static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     bool vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
-    if (MASK == 2 && (reinterpret_cast<uintptr_t>(occ) & 3) != 0) {
-        set_error("invalid argument: occupied_bits is not 4-byte aligned");
-        return CCL_INVALID_ARG;
-    }
     if (vec) CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, true>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate));
     else     CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, false>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate));
     count_launch();
     return CCL_OK;
 }
 
+static int launch_flatten(int64_t n_sites, int32_t* labels, int64_t lo, int64_t hi, const BucketHeader* hdr, int gate,
+                          cudaStream_t st)
+{
+    const int64_t blocks = (((n_sites - lo + 3) / 4) + kThreads - 1) / kThreads;
+    const cudaError_t e = launch_pdl(k_flatten, (unsigned)blocks, (unsigned)kThreads, st, n_sites, labels, lo, hi, hdr, gate);
+    if (e != cudaSuccess) { set_error("launch of k_flatten failed: %s", cudaGetErrorString(e)); return CCL_CUDA_ERROR; }
+    count_launch();
+    return CCL_OK;
+}
+
 template <int MASK>
 static int launch_two_pass(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                           int32_t* labels, const BucketHeader* hdr, const int32_t* gate, cudaStream_t st)
+                           int32_t* labels, const BucketHeader* hdr, int gate, cudaStream_t st)
 {
     const int64_t groups = (n_bonds + 3) / 4;
     int64_t blocks = (groups + kThreads - 1) / kThreads;
@@ -314,27 +365,37 @@ static int launch_two_pass(int64_t n_sites, int64_t n_bonds, const int32_t* src,
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     int vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
-    if (MASK == 2 && (reinterpret_cast<uintptr_t>(occ) & 3) != 0) {
-        set_error("invalid argument: occupied_bits is not 4-byte aligned");
-        return CCL_INVALID_ARG;
-    }
-    const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
-    CCL_CUDA_TRY(launch_pdl(k_hook<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, gate));   // step (i), paper form
+    // hook and the mid-call flatten are this form's own steps (i)/(ii); the join pass also serves as the safety net of
+    // the bucketed form (it joins whatever the ends of an occupied bond still differ in)
+    const int own = gate == kGateNone ? kGateNone : kGateDirect;
+    CCL_CUDA_TRY(launch_pdl(k_hook<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, own));   // step (i), paper form
     count_launch();
-    CCL_CUDA_TRY(launch_pdl(k_flatten, (unsigned)site_blocks, (unsigned)kThreads, st, n_sites, labels, hdr, gate));                   // step (ii)
-    count_launch();
+    { const int rc = launch_flatten(n_sites, labels, 0, n_sites, hdr, own, st); if (rc != CCL_OK) return rc; }                      // step (ii)
     CCL_CUDA_TRY(launch_pdl(k_join<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, gate));   // step (iii)
     count_launch();
+    return CCL_OK;
+}
+
+// Step (ii)/(iv) over the whole array.  windowed: gather from one L2-resident window at a time (see k_flatten).
+static int flatten_all(int64_t n_sites, int32_t* labels, bool windowed, const Tuning& t, cudaStream_t st)
+{
+    int64_t w = n_sites;
+    if (windowed && t.flatten_window_min_bytes >= 0 && n_sites * (int64_t)sizeof(int32_t) >= t.flatten_window_min_bytes) {
+        w = t.flatten_window_bytes / (int64_t)sizeof(int32_t);
+        if (w < 1024) w = 1024;
+        w &= ~(int64_t)3;
+    }
+    for (int64_t lo = 0; lo < n_sites; lo += w) {
+        const int rc = launch_flatten(n_sites, labels, lo, lo + w < n_sites ? lo + w : n_sites, nullptr, kGateNone, st);
+        if (rc != CCL_OK) return rc;
+    }
     return CCL_OK;
 }
 
 // step (ii)/(iv) for the other translation units (ccl_nn.cu)
 int flatten_labels(int64_t n_sites, int32_t* labels, cudaStream_t st)
 {
-    const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
-    k_flatten<<<(unsigned)site_blocks, kThreads, 0, st>>>(n_sites, labels, nullptr, nullptr);
-    CCL_CHECK_LAUNCH("k_flatten");
-    return CCL_OK;
+    return flatten_all(n_sites, labels, false, tuning(), st);
 }
 
 // Optional per-step CUDA events (ccl_set_profile_events): recorded on the call's stream between the kernels so
@@ -346,77 +407,122 @@ static inline void mark(int k, cudaStream_t st)
     if (g_ev[k]) cudaEventRecord(g_ev[k], st);
 }
 
+// ---- what the region probe said about a bond list, remembered on the host ----------------------------------------
+// Both forms of step (iii) are correct for every graph; the probe only picks the faster one.  The first call on a
+// bond list enqueues both behind the device-side probe and copies the probe's answer to pinned host memory; later
+// calls on the same (src, dst, n_bonds, n_sites) -- an occupancy sweep, the paper's use -- enqueue only the chosen form
+// and can then fold step (i) into the bucketed kernels.  A stale entry (the caller rewrote the arrays) costs speed only.
+struct ProbeHint {
+    const void* src = nullptr;
+    const void* dst = nullptr;
+    int64_t n_bonds = 0, n_sites = 0;
+    int shift = 0;
+    int32_t* answer = nullptr;                     // pinned; -1 until the copy has landed
+};
+static thread_local ProbeHint g_hints[4];
+static thread_local int g_hint_next = 0;
+
+static ProbeHint* hint_find(const void* src, const void* dst, int64_t n_bonds, int64_t n_sites, int shift)
+{
+    for (ProbeHint& h : g_hints)
+        if (h.answer && h.src == src && h.dst == dst && h.n_bonds == n_bonds && h.n_sites == n_sites && h.shift == shift) return &h;
+    return nullptr;
+}
+
+static ProbeHint* hint_new(const void* src, const void* dst, int64_t n_bonds, int64_t n_sites, int shift)
+{
+    ProbeHint& h = g_hints[g_hint_next];
+    g_hint_next = (g_hint_next + 1) % 4;
+    if (h.answer == nullptr && cudaHostAlloc(reinterpret_cast<void**>(&h.answer), sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) {
+        h.answer = nullptr;
+        cudaGetLastError();
+        return nullptr;
+    }
+    *reinterpret_cast<volatile int32_t*>(h.answer) = -1;
+    h.src = src; h.dst = dst; h.n_bonds = n_bonds; h.n_sites = n_sites; h.shift = shift;
+    return &h;
+}
+
 static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
                       int mask_kind, int32_t* labels, cudaStream_t st)
 {
     int rc = check_args(n_sites, n_bonds, src, dst, labels);
     if (rc != CCL_OK) return rc;
     if (n_sites == 0) return CCL_OK;
-    const bool lab_vec = (reinterpret_cast<uintptr_t>(labels) & 15) == 0;
-    if (!lab_vec) { set_error("labels must be 16-byte aligned"); return CCL_UNSUPPORTED; }
+    CCL_REQUIRE((reinterpret_cast<uintptr_t>(labels) & 15) == 0, "labels must be 16-byte aligned");
+    CCL_REQUIRE(mask_kind != 2 || (reinterpret_cast<uintptr_t>(occ) & 3) == 0, "occupied_bits is not 4-byte aligned");
+    const Tuning t = tuning();                             // one snapshot per call
 
-    const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
-    // Tiled form (ccl_tile.cu): steps (i)-(iii) with the label reduction in shared memory, for bond lists that are local
-    // in the site numbering.  A device-side probe decides; the kernels of the other forms are enqueued behind it and
-    // return at once when it did the work (*gate == 0), so no decision ever needs a host round trip.
-    int tiled = kTiledNo;
-    const int32_t* gate = nullptr;
-    void* tile_ws = nullptr;
-    rc = tiled_reduce(n_sites, n_bonds, src, dst, occ, mask_kind, labels, st, &tiled, &gate, &tile_ws);
-    if (rc != CCL_OK) return rc;
-    auto done = [&](int code) { if (tile_ws) cudaFreeAsync(tile_ws, st); return code; };
-    if (tiled == kTiledFinal) { mark(0, st); mark(1, st); mark(2, st); return CCL_OK; }
-    void* bucket_ws = nullptr;
+    // Which form of step (iii)?  0 = direct kernels, 1 = region-bucketed, -1 = a device-side probe decides.
+    int mode = 0;
     BucketPlan plan;
-    ProbeJob job;
-    auto done2 = [&](int code) { if (bucket_ws) cudaFreeAsync(bucket_ws, st); return done(code); };
-    if (tiled != kTiledForced) {
-        // Label arrays that cannot stay in L2 get the region-bucketed form if a device-side probe finds the bonds
-        // non-local in the site numbering; the direct kernel then returns at once (and vice versa).
-        if (n_bonds > 0 && tuning().force_mode != 0 && n_sites * (int64_t)sizeof(int32_t) >= tuning().bucket_min_label_bytes &&
-            n_bonds >= tuning().bucket_min_bonds) {
-            rc = bucketed_begin(n_sites, n_bonds, src, dst, st, &plan, &job, &bucket_ws);
-            if (rc != CCL_OK) return done2(rc);
-        }
-        const int64_t init_blocks = site_blocks < (int64_t)kSMs * 32 ? site_blocks : (int64_t)kSMs * 32;
-        k_init<<<(unsigned)init_blocks, kThreads, 0, st>>>(n_sites, labels, gate, job);         // step (i) (+ the probe)
-        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_init failed: %s", cudaGetErrorString(e)); return done2(CCL_CUDA_ERROR); } count_launch(); }
-    }
-    // step (ii): nothing to do after label[i] = i (every site is a root).
-    mark(0, st);
-    if (n_bonds > 0) {
-        if (tiled != kTiledForced) {
-            // step (iii)
-            BucketHeader* hdr = plan.hdr;
-            if (hdr != nullptr) {
-                rc = bucketed_launch(plan, n_bonds, src, dst, occ, mask_kind, labels, st);
-                if (rc != CCL_OK) return done2(rc);
+    void* bucket_ws = nullptr;
+    ProbeHint* hint = nullptr;
+    bool report_probe = false;
+    const bool eligible = n_bonds > 0 && t.force_mode != 0 && n_sites * (int64_t)sizeof(int32_t) >= t.bucket_min_label_bytes &&
+                          n_bonds >= t.bucket_min_bonds;
+    if (eligible) {
+        rc = bucketed_begin(n_sites, n_bonds, t, st, &plan, &bucket_ws);
+        if (rc != CCL_OK) return rc;
+        mode = t.force_mode == 1 ? 1 : -1;
+        if (mode < 0 && t.probe_cache) {
+            hint = hint_find(src, dst, n_bonds, n_sites, plan.shift);
+            if (hint) {
+                const int32_t ans = *reinterpret_cast<volatile int32_t*>(hint->answer);
+                if (ans == 0 || ans == 1) mode = ans;
+            } else {
+                hint = hint_new(src, dst, n_bonds, n_sites, plan.shift);
+                report_probe = hint != nullptr;
             }
-            // Two passes pay where most bonds close cycles (many bonds per site: triangular lattice 0.70 -> 0.53 ms);
-            // with 1.5-2 bonds per site (honeycomb, random regular graphs) they are neutral or slower.
-            const bool two_pass = tuning().two_pass > 0 ||
-                                  (tuning().two_pass < 0 && n_bonds >= (1 << 20) && 2 * n_bonds >= 5 * n_sites);
-            if (two_pass) {
-                if (occ == nullptr) rc = launch_two_pass<0>(n_sites, n_bonds, src, dst, nullptr, labels, hdr, gate, st);
-                else if (mask_kind == 1) rc = launch_two_pass<1>(n_sites, n_bonds, src, dst, occ, labels, hdr, gate, st);
-                else rc = launch_two_pass<2>(n_sites, n_bonds, src, dst, occ, labels, hdr, gate, st);
-            } else if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, hdr, gate, st);
-            else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, hdr, gate, st);
-            else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, hdr, gate, st);
-            if (rc != CCL_OK) return done2(rc);
         }
-        mark(1, st);
-        {                                                                                       // step (iv)
-            const cudaError_t e = launch_pdl(k_flatten, (unsigned)site_blocks, (unsigned)kThreads, st, n_sites, labels,
-                                             (const BucketHeader*)nullptr, (const int32_t*)nullptr);
-            if (e != cudaSuccess) { set_error("launch of k_flatten failed: %s", cudaGetErrorString(e)); return done2(CCL_CUDA_ERROR); }
-            count_launch();
-        }
-        mark(2, st);
     }
-    if (bucket_ws) cudaFreeAsync(bucket_ws, st);
-    if (tile_ws) cudaFreeAsync(tile_ws, st);
-    return CCL_OK;
+    auto done = [&](int code) { if (bucket_ws) cudaFreeAsync(bucket_ws, st); return code; };
+    const int gate = mode < 0 ? kGateDirectOrOverflow : kGateOverflow;
+
+    // ---- step (i); step (ii) has nothing to do after label[i] = i (every site is a root)
+    if (mode != 1) {
+        ProbeJob job;
+        if (mode < 0) { job.hdr = plan.hdr; job.n_bonds = n_bonds; job.src = src; job.dst = dst; job.shift = plan.shift; }
+        const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
+        const int64_t init_blocks = site_blocks < (int64_t)kSMs * 32 ? site_blocks : (int64_t)kSMs * 32;
+        k_init<<<(unsigned)init_blocks, kThreads, 0, st>>>(n_sites, labels, job);                // (+ the probe)
+        { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_init failed: %s", cudaGetErrorString(e)); return done(CCL_CUDA_ERROR); } count_launch(); }
+        mark(0, st);
+    }
+    if (n_bonds > 0) {
+        // ---- step (iii)
+        if (mode != 0) {
+            plan.lazy_init = mode == 1;                    // step (i) region by region inside the bucketed kernels
+            plan.gated = mode < 0;
+            if (mode == 1) mark(0, st);                    // no separate initialization pass to time
+            rc = bucketed_launch(plan, n_sites, n_bonds, src, dst, occ, mask_kind, labels, st);
+            if (rc != CCL_OK) return done(rc);
+        }
+        // The direct kernels: the whole of step (iii) in direct mode; behind the bucketed kernels they return at once
+        // unless the probe chose them (mode < 0) or the chunk pool ran dry.  Two passes pay where most bonds close
+        // cycles (many bonds per site: triangular lattice); with 1.5-2 bonds per site they are neutral or slower.
+        const BucketHeader* hdr = mode != 0 ? plan.hdr : nullptr;
+        const int g = mode != 0 ? gate : kGateNone;
+        const bool two_pass = mode != 1 && (t.two_pass > 0 || (t.two_pass < 0 && n_bonds >= (1 << 20) && 2 * n_bonds >= 5 * n_sites));
+        if (two_pass) {
+            if (occ == nullptr) rc = launch_two_pass<0>(n_sites, n_bonds, src, dst, nullptr, labels, hdr, g, st);
+            else if (mask_kind == 1) rc = launch_two_pass<1>(n_sites, n_bonds, src, dst, occ, labels, hdr, g, st);
+            else rc = launch_two_pass<2>(n_sites, n_bonds, src, dst, occ, labels, hdr, g, st);
+        } else if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, hdr, g, st);
+        else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, hdr, g, st);
+        else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, hdr, g, st);
+        if (rc != CCL_OK) return done(rc);
+        mark(1, st);
+        // ---- step (iv)
+        rc = flatten_all(n_sites, labels, mode != 0, t, st);
+        if (rc != CCL_OK) return done(rc);
+        mark(2, st);
+        if (report_probe && cudaMemcpyAsync(hint->answer, &plan.hdr->mode, sizeof(int32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess)
+            cudaGetLastError();                            // a hint only
+    } else {
+        mark(1, st); mark(2, st);
+    }
+    return done(CCL_OK);
 }
 
 }  // namespace ccl
@@ -473,26 +579,30 @@ extern "C" int ccl_label_bits_host(int64_t n_sites, int64_t n_bonds, const int32
     const size_t label_bytes = (size_t)n_sites * sizeof(int32_t);
     int32_t *d_src = nullptr, *d_dst = nullptr, *d_labels = nullptr;
     uint32_t* d_bits = nullptr;
-    if ((rc = scratch_alloc((void**)&d_labels, label_bytes, st)) != CCL_OK) return rc;
-    if (n_bonds > 0) {
-        if ((rc = scratch_alloc((void**)&d_src, bond_bytes, st)) != CCL_OK) return rc;
-        if ((rc = scratch_alloc((void**)&d_dst, bond_bytes, st)) != CCL_OK) return rc;
-        CCL_CUDA_TRY(cudaMemcpyAsync(d_src, host_src, bond_bytes, cudaMemcpyHostToDevice, st));
-        CCL_CUDA_TRY(cudaMemcpyAsync(d_dst, host_dst, bond_bytes, cudaMemcpyHostToDevice, st));
-        if (mask_bytes) {
-            if ((rc = scratch_alloc((void**)&d_bits, mask_bytes, st)) != CCL_OK) return rc;
-            CCL_CUDA_TRY(cudaMemcpyAsync(d_bits, host_occupied_bits, mask_bytes, cudaMemcpyHostToDevice, st));
+    auto run = [&]() -> int {                              // every exit goes through the one cleanup below
+        int r;
+        if ((r = scratch_alloc((void**)&d_labels, label_bytes, st)) != CCL_OK) return r;
+        if (n_bonds > 0) {
+            if ((r = scratch_alloc((void**)&d_src, bond_bytes, st)) != CCL_OK) return r;
+            if ((r = scratch_alloc((void**)&d_dst, bond_bytes, st)) != CCL_OK) return r;
+            CCL_CUDA_TRY(cudaMemcpyAsync(d_src, host_src, bond_bytes, cudaMemcpyHostToDevice, st));
+            CCL_CUDA_TRY(cudaMemcpyAsync(d_dst, host_dst, bond_bytes, cudaMemcpyHostToDevice, st));
+            if (mask_bytes) {
+                if ((r = scratch_alloc((void**)&d_bits, mask_bytes, st)) != CCL_OK) return r;
+                CCL_CUDA_TRY(cudaMemcpyAsync(d_bits, host_occupied_bits, mask_bytes, cudaMemcpyHostToDevice, st));
+            }
         }
-    }
-    rc = label_impl(n_sites, n_bonds, d_src, d_dst, d_bits, 2, d_labels, st);
-    if (rc == CCL_OK) {
+        if ((r = label_impl(n_sites, n_bonds, d_src, d_dst, d_bits, 2, d_labels, st)) != CCL_OK) return r;
         CCL_CUDA_TRY(cudaMemcpyAsync(host_labels, d_labels, label_bytes, cudaMemcpyDeviceToHost, st));
-    }
+        return CCL_OK;
+    };
+    rc = run();
     if (d_bits) cudaFreeAsync(d_bits, st);
     if (d_dst) cudaFreeAsync(d_dst, st);
     if (d_src) cudaFreeAsync(d_src, st);
-    cudaFreeAsync(d_labels, st);
-    CCL_CUDA_TRY(cudaStreamSynchronize(st));
+    if (d_labels) cudaFreeAsync(d_labels, st);
+    const cudaError_t e = cudaStreamSynchronize(st);
+    if (rc == CCL_OK && e != cudaSuccess) { set_error("cudaStreamSynchronize failed: %s", cudaGetErrorString(e)); rc = CCL_CUDA_ERROR; }
     return rc;
 }
 
@@ -519,6 +629,7 @@ extern "C" int ccl_label_sweep_host(int64_t n_sites, int64_t n_bonds, const int3
     cudaStream_t side = nullptr;
     cudaEvent_t labeled[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
     auto cleanup = [&]() {
+        if (side) cudaStreamSynchronize(side);            // a copy may still be reading a label buffer
         for (int j = 0; j < 2; ++j) {
             if (d_bits[j]) cudaFreeAsync(d_bits[j], st);
             if (d_labels[j]) cudaFreeAsync(d_labels[j], st);

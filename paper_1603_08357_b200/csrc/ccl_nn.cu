@@ -8,8 +8,9 @@
 //                other lower-numbered neighbours) is not stored: it is re-read from the NN list in step (iii).  No
 //                atomics: every site writes its own label.
 //   k_flatten    step (ii): analysis (ccl_label.cu).
-//   k_nn_reduce  step (iii): for every site i and every lower-numbered neighbour j: Algorithm 1 on
-//                (i, j).  The labels are flat after (ii), so most pairs are seen to be joined by two reads.
+//   k_nn_reduce  step (iii): for every site i and every listed neighbour j != i: Algorithm 1 on
+//                (i, j).  The labels are flat after (ii), so most pairs are seen to be joined by two reads.  (A bond
+//                may be listed at its lower end only; step (i) does not see it there, step (iii) joins it.)
 //   k_flatten    step (iv).
 //
 // Product code: nothing under oracle/ is included here or includes this.
@@ -47,7 +48,10 @@ k_nn_reduce(int64_t n_sites, int z_max, const int32_t* __restrict__ nn, int32_t*
             const int32_t j = live ? nn[(int64_t)k * n_sites + i] : -1;
             bool need = false;
             int32_t la = 0, lb = 0;
-            if (j >= 0 && j < (int32_t)i) {                                // the residual list: lower-numbered neighbours
+            // Every entry is a bond, whichever end lists it (include/ccl.h).  Lower-numbered neighbours are the paper's
+            // residual list; an entry j > i joins the same way (Algorithm 1 is symmetric) -- if the list also names the
+            // bond at site j, the second look finds the two labels equal and costs two reads.
+            if (j >= 0 && j != (int32_t)i) {
                 la = ld_label(label + i);
                 lb = ld_label(label + j);
                 need = la != lb;

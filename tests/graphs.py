@@ -156,14 +156,20 @@ def same_partition(a, b):
     return True
 
 
-def nn_list_from_bonds(n_sites, src, dst, occupied=None, both_sides=True):
+def nn_list_from_bonds(n_sites, src, dst, occupied=None, both_sides=True, rng=None):
     """Dense z_max x n_sites nearest-neighbour list (structure of arrays, -1 padding) of the occupied bonds.
-    both_sides: each bond is listed at both of its ends (the paper's form) or only at its higher-numbered end."""
+    both_sides: True = each bond is listed at both of its ends (the paper's form); False or "higher" = only at its
+    higher-numbered end; "lower" = only at its lower-numbered end; "random" = at one end chosen by rng per bond."""
     keep = np.ones(len(src), dtype=bool) if occupied is None else np.asarray(occupied) != 0
     u = np.asarray(src)[keep].astype(np.int64)
     v = np.asarray(dst)[keep].astype(np.int64)
-    if both_sides:
+    if both_sides is True:
         a, b = np.concatenate([u, v]), np.concatenate([v, u])
+    elif both_sides == "lower":
+        a, b = np.minimum(u, v), np.maximum(u, v)
+    elif both_sides == "random":
+        flip = rng.random(u.size) < 0.5
+        a, b = np.where(flip, u, v), np.where(flip, v, u)
     else:
         a, b = np.maximum(u, v), np.minimum(u, v)
     order = np.argsort(a, kind="stable")

@@ -41,6 +41,10 @@ def test_argument_checking_is_host_side():
     assert lib.ccl_label(4, 3, p, p, None, None, None) == 1
     assert lib.ccl_label_bits(4, 3, p, None, None, p, None) == 1
     assert lib.ccl_label(0, 0, None, None, None, None, None) == 0            # empty graph: no-op
+    assert lib.ccl_label(4, 0, None, None, None, ((p + 15) & ~15) + 4, None) == 1    # labels must be 16-byte aligned
+    assert "16-byte" in binding.last_error()
+    assert lib.ccl_set_option(b"no_such_option", 1) == 1
+    assert lib.ccl_set_option(b"scatter_tiles", 0) == 0 and lib.ccl_set_option(b"reset", 0) == 0
     assert lib.ccl_gen_triangular(0, p, p, None) == 1
     assert lib.ccl_gen_honeycomb(40000, p, p, None) == 1                      # 2 L^2 > 2^31-1
     assert lib.ccl_gen_occupancy(8, -0.5, 1, 0, p, None, None) == 1

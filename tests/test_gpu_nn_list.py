@@ -31,15 +31,16 @@ def test_fig1_nn_list_gives_fig4_labels(ccl):
     assert ccl.label_nn(dev(arr)).cpu().tolist() == want["fig4_right"]
 
 
-@pytest.mark.parametrize("both_sides", [True, False])
+@pytest.mark.parametrize("both_sides", [True, False, "lower", "random"])
 def test_random_graphs(ccl, both_sides):
-    rng = np.random.default_rng(111 + both_sides)
+    """include/ccl.h: every entry is a connection, listed from one side or from both -- whichever side."""
+    rng = np.random.default_rng(111 + [True, False, "lower", "random"].index(both_sides))
     for trial in range(40):
         n = int(rng.integers(1, 30000))
         m = int(rng.integers(0, 3 * n + 1))
         src, dst = graphs.random_graph(rng, n, m, self_loops=True)
         mask = (rng.random(m) < rng.random()).astype(np.uint8)
-        nn = graphs.nn_list_from_bonds(n, src, dst, mask, both_sides)
+        nn = graphs.nn_list_from_bonds(n, src, dst, mask, both_sides, rng)
         got = ccl.label_nn(dev(nn).reshape(nn.shape[0], n)).cpu().numpy()
         want = oracle.label(n, src, dst, mask) if m else np.arange(n, dtype=np.int32)
         assert np.array_equal(got, want)
@@ -66,6 +67,8 @@ def test_cayley_tree_and_paths(ccl):
     rng = np.random.default_rng(8)
     for order in ("ascending", "descending", "shuffled"):
         s, d = graphs.path_graph(1 << 18, order, rng)
-        assert int(ccl.label_nn(dev(graphs.nn_list_from_bonds(1 << 18, s, d))).max().item()) == 0
+        for sides in (True, "lower"):
+            got = ccl.label_nn(dev(graphs.nn_list_from_bonds(1 << 18, s, d, None, sides)))
+            assert int(got.max().item()) == 0 and int(got.min().item()) == 0
     empty = torch.zeros((0, 9), dtype=torch.int32, device="cuda")
     assert ccl.label_nn(empty).cpu().tolist() == list(range(9))

@@ -25,6 +25,11 @@ def dev(a, dtype=None):
     return t.cuda()
 
 
+def all_zero(t):
+    """Every label is 0: the maximum alone would miss a negative label."""
+    return int(t.max().item()) == 0 and int(t.min().item()) == 0
+
+
 def bits_dev(bits):
     return dev(bits.view(np.int32))
 
@@ -108,17 +113,17 @@ def test_path_graph_worst_case_depth(ccl, order):
     n = 1 << 20
     src, dst = graphs.path_graph(n, order, rng)
     got = ccl.label(n, dev(src), dev(dst))
-    assert int(got.max().item()) == 0
+    assert int(got.max().item()) == 0 and int(got.min().item()) == 0
     perm = rng.permutation(src.size)
     got = ccl.label(n, dev(src[perm]), dev(dst[perm]))
-    assert int(got.max().item()) == 0
+    assert int(got.max().item()) == 0 and int(got.min().item()) == 0
 
 
 def test_star_and_clique_contention(ccl):
     n = 1 << 16
     hub = np.full(n - 1, n - 1, dtype=np.int32)              # every bond hits the highest-numbered site
     leaves = np.arange(n - 1, dtype=np.int32)
-    assert int(ccl.label(n, dev(hub), dev(leaves)).max().item()) == 0
+    assert all_zero(ccl.label(n, dev(hub), dev(leaves)))
     k = 300
     iu = np.triu_indices(k, 1)
     src, dst = iu[1].astype(np.int32) + 5, iu[0].astype(np.int32) + 5
@@ -231,23 +236,16 @@ def test_host_buffer_sweep_entry_point(ccl):
 # ------------------------------------------------------------------ region-bucketed form of step (iii)
 @pytest.fixture
 def bucketed(ccl):
-    """Force the bucketed form on small inputs: every call eligible, 2^10..2^14-site regions.  set_tuning() resets all
-    options, so the tiled form (which would take these calls first) is switched off after each set_tuning call."""
-    class Off:
-        def __getattr__(self, name):
-            return getattr(ccl, name)
-
-        def set_tuning(self, *a):
-            ccl.set_tuning(*a)
-            ccl.set_option("tile_mode", 0)
-    yield Off()
+    """Force the bucketed form on small inputs: every call eligible, 2^10..2^14-site regions."""
+    yield ccl
     ccl.set_tuning()                                   # restore defaults
 
 
-@pytest.mark.parametrize("shift,cap", [(10, 0), (12, 0), (14, 0), (12, 64), (16, 1000)])
+@pytest.mark.parametrize("shift,cap", [(10, 0), (12, 0), (14, 0), (12, 64), (16, 1000), (11, 20000)])
 def test_bucketed_form_random_small_graphs(bucketed, shift, cap):
     ccl = bucketed
-    ccl.set_tuning(0, shift, 1, cap)                   # cap > 0: tiny buckets, most pairs take the overflow path
+    ccl.set_tuning(0, shift, 1, cap)                   # cap > 0: a pool of one to three chunks; when it runs dry the pairs are
+                                                       # dropped and the direct kernel redoes the bond list behind the descent
     rng = np.random.default_rng(shift * 131 + cap)
     for trial in range(40):
         n = int(rng.integers(2, 60000))
@@ -277,10 +275,10 @@ def test_bucketed_form_adversarial(bucketed):
     n = 1 << 17
     for order in ("ascending", "descending", "shuffled"):
         src, dst = graphs.path_graph(n, order, rng)
-        assert int(ccl.label(n, dev(src), dev(dst)).max().item()) == 0
+        assert all_zero(ccl.label(n, dev(src), dev(dst)))
     hub = np.full(n - 1, n - 1, dtype=np.int32)        # star on the highest site: every pair lands in one bucket
     leaves = np.arange(n - 1, dtype=np.int32)
-    assert int(ccl.label(n, dev(hub), dev(leaves)).max().item()) == 0
+    assert all_zero(ccl.label(n, dev(hub), dev(leaves)))
     # interleaved path 0, n/2, 1, n/2+1, ...: every bond crosses regions and the lower half becomes one long chain
     half = n // 2
     i = np.arange(half - 1, dtype=np.int32)
@@ -290,104 +288,16 @@ def test_bucketed_form_adversarial(bucketed):
     assert np.array_equal(got, oracle.label(n, src, dst))
 
 
-# ------------------------------------------------------------------ tiled form: label reduction in shared memory
 @pytest.fixture
-def tiled(ccl):
+def options(ccl):
     yield ccl
     ccl.set_option("reset")
 
 
-def _tile_opts(ccl, sub_shift, tile_mode=1, fine_cap=0, small=0, min_bonds=0):
-    """tile_mode 1: the tiled kernels run whatever the probe would say; -1: the device-side probe decides and the other
-    forms run behind the same flag.  small = 0 switches the one-CTA kernel off so that small inputs reach k_local."""
-    ccl.set_option("reset")
-    ccl.set_option("tile_mode", tile_mode)
-    ccl.set_option("sub_shift", sub_shift)
-    ccl.set_option("fine_capacity", fine_cap)
-    ccl.set_option("small_max_sites", small)
-    ccl.set_option("tile_min_bonds", min_bonds)
-
-
-@pytest.mark.parametrize("sub_shift,tile_mode,fine_cap", [
-    (4, 1, 0), (6, 1, 0), (6, -1, 0), (10, 1, 0), (10, -1, 0),
-    (8, 1, 16),                 # tiny window buckets: most pairs take the overflow list
-    (15, 1, 0), (-1, 1, 0), (-1, -1, 0)])
-def test_tiled_form_random_small_graphs(tiled, sub_shift, tile_mode, fine_cap):
-    ccl = tiled
-    _tile_opts(ccl, sub_shift, tile_mode, fine_cap)
-    rng = np.random.default_rng(1000 + sub_shift * 7 + tile_mode + fine_cap)
-    for trial in range(30):
-        # at most 2048 windows: larger n would fall through to the other forms
-        n = int(rng.integers(2, min(2000 << max(sub_shift - 4, 0), 300000))) if sub_shift >= 0 else int(rng.integers(2, 100000))
-        m = int(rng.integers(1, 3 * n + 1))
-        src, dst = graphs.random_graph(rng, n, m, self_loops=True)
-        if trial % 3 == 0:                                  # local bonds: the probe picks the tiled form
-            dst = np.clip(src + rng.integers(-3, 4, size=m), 0, n - 1).astype(np.int32)
-        mask = (rng.random(m) < rng.random()).astype(np.uint8)
-        run_all_forms(ccl, n, src, dst, mask)
-        assert np.array_equal(ccl.label(n, dev(src), dev(dst)).cpu().numpy(), oracle.label(n, src, dst))
-
-
-def test_one_cta_kernel_small_graphs(tiled):
-    ccl = tiled
-    ccl.set_option("reset")
-    ccl.set_option("tile_mode", -1)                         # tiled forms on: n_sites <= 2^15 takes k_small
-    rng = np.random.default_rng(4242)
-    for trial in range(40):
-        n = int(rng.integers(1, 1 << 15)) if trial else 1 << 15
-        m = int(rng.integers(1, 3 * n + 1))
-        src, dst = graphs.random_graph(rng, n, m, self_loops=True)
-        if trial % 2:
-            dst = np.clip(src + rng.integers(-2, 3, size=m), 0, n - 1).astype(np.int32)
-        mask = (rng.random(m) < rng.random()).astype(np.uint8)
-        run_all_forms(ccl, n, src, dst, mask)
-
-
-@pytest.mark.parametrize("name", ["cfg1_honeycomb_L64", "honeycomb_L301", "triangular_L257", "regular3", "regular4",
-                                  "cayley_standard", "cayley_random"])
-@pytest.mark.parametrize("sub_shift,tile_mode", [(-1, -1), (9, 1), (12, -1), (15, 1)])
-def test_tiled_form_workloads_bit_exact(tiled, name, sub_shift, tile_mode):
-    ccl = tiled
-    n, src, dst, ps, cfg = _case(name)
-    _tile_opts(ccl, sub_shift, tile_mode)
-    for p in ps + [1.0]:
-        mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(cfg), realization=3)
-        run_all_forms(ccl, n, src, dst, mask)
-
-
-def test_tiled_form_adversarial(tiled):
-    ccl = tiled
-    rng = np.random.default_rng(77)
-    n = 1 << 17
-    for sub_shift, tile_mode in [(8, 1), (12, -1), (15, 1)]:
-        _tile_opts(ccl, sub_shift, tile_mode)
-        for order in ("ascending", "descending", "shuffled"):
-            src, dst = graphs.path_graph(n, order, rng)
-            assert int(ccl.label(n, dev(src), dev(dst)).max().item()) == 0
-        hub = np.full(n - 1, n - 1, dtype=np.int32)    # star on the highest site: one window takes every pair
-        leaves = np.arange(n - 1, dtype=np.int32)
-        assert int(ccl.label(n, dev(hub), dev(leaves)).max().item()) == 0
-        same = np.full(5000, n - 3, dtype=np.int32)    # 5000 copies of one bond
-        assert ccl.label(n, dev(same), dev(np.full(5000, 7, dtype=np.int32))).cpu().numpy()[n - 3] == 7
-        half = n // 2
-        i = np.arange(half - 1, dtype=np.int32)
-        src = np.concatenate([i, i + half]).astype(np.int32)
-        dst = np.concatenate([i + half, i + 1]).astype(np.int32)
-        got = ccl.label(n, dev(src), dev(dst)).cpu().numpy()
-        assert np.array_equal(got, oracle.label(n, src, dst))
-        # a comb: long local chains inside every window plus one long-range bond per window (residue list)
-        step = 1 << sub_shift
-        src = np.concatenate([np.arange(n - 1), np.arange(0, n - step, step)]).astype(np.int32)
-        dst = np.concatenate([np.arange(1, n), np.arange(step, n, step) + 1]).astype(np.int32)
-        mask = (rng.random(src.size) < 0.97).astype(np.uint8)
-        got = ccl.label(n, dev(src), dev(dst), dev(mask)).cpu().numpy()
-        assert np.array_equal(got, oracle.label(n, src, dst, mask))
-
-
 # ------------------------------------------------------------------ two-pass direct form (hook, flatten, join)
 @pytest.mark.parametrize("two_pass", [0, 1])
-def test_two_pass_form(tiled, two_pass):
-    ccl = tiled
+def test_two_pass_form(options, two_pass):
+    ccl = options
     ccl.set_option("reset")
     ccl.set_option("two_pass", two_pass)
     rng = np.random.default_rng(31 + two_pass)
@@ -405,7 +315,7 @@ def test_two_pass_form(tiled, two_pass):
     n = 1 << 18
     for order in ("ascending", "descending", "shuffled"):
         src, dst = graphs.path_graph(n, order, rng)
-        assert int(ccl.label(n, dev(src), dev(dst)).max().item()) == 0
+        assert all_zero(ccl.label(n, dev(src), dev(dst)))
 
 
 def test_tuning_argument_checks(ccl):
@@ -434,8 +344,10 @@ def test_no_write_outside_the_label_buffer(ccl):
         def intact(buf):
             return bool((buf[:GUARD] == MAGIC).all().item()) and bool((buf[GUARD + n:] == MAGIC).all().item())
 
-        for opts in ({}, {"two_pass": 1}, {"tile_mode": 1, "small_max_sites": 0}, {"tile_mode": -1},
-                     {"bucket_min_label_bytes": 0, "region_shift": 10, "force_mode": 1}):
+        for opts in ({}, {"two_pass": 1}, {"flatten_window_min_bytes": 0, "flatten_window_bytes": 4096},
+                     {"bucket_min_label_bytes": 0, "region_shift": 10, "force_mode": 1},
+                     {"bucket_min_label_bytes": 0, "region_shift": 10, "scatter_tiles": 0},
+                     {"bucket_min_label_bytes": 0, "region_shift": 10, "bucket_capacity": 100, "flatten_window_bytes": 8192}):
             ccl.set_option("reset")
             for k, v in opts.items():
                 ccl.set_option(k, v)
