@@ -42,7 +42,7 @@ WORKLOADS = {
 }
 METRIC = "Gbonds/s labeled (1 B200) and achieved HBM GB/s fraction of roofline"
 SEED_BASE = 0x1603083570000000          # DESIGN.md input recipe: seed = SEED_BASE + config number
-CPU_SAMPLE_LOG2_SITES = 22              # cpu_baseline / reference arm: same family at 2^22 sites (bounded sample)
+CPU_BUDGET_S = 150.0                    # reference arm: labeling time it may spend (steps are cut to fit, never the graph)
 
 
 def describe(name):
@@ -134,46 +134,62 @@ class ClockSampler:
         return out
 
 
-def cpu_oracle_sample(name, steps, warmup):
-    """The oracle as it stands, single thread, on a bounded sample of the workload; returns (Gbonds/s, seconds per
-    step, description).  Lattice workloads are sampled at L = 1024, the regular graphs at 2^22 sites."""
-    import numpy as np  # noqa: F401
+def oracle_inputs(name, realization=0):
+    """The configured workload from the oracle's own CPU generators (untimed): (n, src, dst, [(mask, bits) per p], text)."""
+    import numpy as np
     from oracle import oracle
     fam, size, z, ps, kind, cfg = WORKLOADS[name]
     seed = SEED_BASE + cfg
     if fam == "regular":
-        n = min(size, 1 << CPU_SAMPLE_LOG2_SITES)
+        n = size
         src, dst, _ = oracle.gen_regular(n, z, seed)
-        sample = "random %d-regular graph, N=2^%d sites, M=%d bonds" % (z, n.bit_length() - 1, src.size)
+        text = "random %d-regular graph, N=2^%d sites, M=%d bonds" % (z, n.bit_length() - 1, src.size)
     elif fam == "cayley":
-        g = min(size, 20)
-        n = 3 * (1 << g) - 2
+        n = 3 * (1 << size) - 2
         perm = np.random.default_rng(seed & 0x7FFFFFFF).permutation(n).astype(np.int32) if z else None
-        n, src, dst = oracle.gen_cayley3(g, perm)
-        sample = "Cayley tree z=3 g=%d (%s numbering), N=%d sites, M=%d bonds" % (g, "random" if z else "standard", n, src.size)
+        n, src, dst = oracle.gen_cayley3(size, perm)
+        text = "Cayley tree z=3 g=%d (%s numbering), N=%d sites, M=%d bonds" % (size, "random" if z else "standard", n, src.size)
     else:
-        L = min(size, 1024)
-        src, dst = (oracle.gen_honeycomb if fam.startswith("honeycomb") else oracle.gen_triangular)(L)
-        n = (2 if fam.startswith("honeycomb") else 1) * L * L
-        sample = "%s L=%d, N=%d sites, M=%d bonds (bond-list oracle)" % (fam, L, n, src.size)
-    reps = 256 if fam == "honeycomb_batch" else 1           # a bounded sample of the batch: 256 realizations per p
-    masks = [oracle.gen_occupancy(src.size, p, seed, r) for p in ps for r in range(reps)]
+        src, dst = (oracle.gen_honeycomb if fam.startswith("honeycomb") else oracle.gen_triangular)(size)
+        n = (2 if fam.startswith("honeycomb") else 1) * size * size
+        text = "%s L=%d, N=%d sites, M=%d bonds" % (fam.split("_")[0], size, n, src.size)
+    reps = 64 if fam == "honeycomb_batch" else 1           # the batch workload: a bounded number of realizations per p
+    masks = [oracle.gen_occupancy(src.size, p, seed, realization * reps + r) for p in ps for r in range(reps)]
     if reps > 1:
-        sample += " x %d realizations" % reps
-    times = []
-    for it in range(warmup + steps):
+        text += " x %d realizations" % reps
+    return n, src, dst, masks, text
+
+
+def time_oracle(name, n, src, dst, masks, steps, warmup, budget_s=None):
+    """The oracle as it stands, one thread, on the configured graph: one step = one labeling per mask of the sweep.  The
+    number of steps (never the graph) is cut so that the timed labelings fit budget_s.  Returns (Gbonds/s, s per step,
+    steps, warmup)."""
+    from oracle import oracle
+    kind = WORKLOADS[name][4]
+
+    def sweep():
         t0 = time.perf_counter()
         for mask, bits in masks:
             if kind == "u8":
                 oracle.label(n, src, dst, mask)
             else:
                 oracle.label_bits(n, src, dst, bits)
-        if it >= warmup:
-            times.append(time.perf_counter() - t0)
+        return time.perf_counter() - t0
+    first = sweep()
+    times = []
+    if budget_s is not None:
+        steps = max(1, min(steps, int(budget_s / max(first, 1e-9))))
+        if first * (steps + 1) > budget_s + first:       # a sweep that takes tens of seconds is its own warm-up
+            warmup = 0
+    if warmup == 0:
+        times.append(first)
+    else:
+        for _ in range(warmup - 1):
+            sweep()
+    while len(times) < steps:
+        times.append(sweep())
     per_step = sum(times) / len(times)
-    sample += ", p sweep " + ",".join("%.4g" % p for p in ps) + ", same seeds; labeling time only (oracle_label%s)" % (
-        "" if kind == "u8" else "_bits")
-    return len(masks) * src.size / per_step / 1e9, per_step, sample
+    return len(masks) * src.size / per_step / 1e9, per_step, len(times), warmup
 
 
 def replica_plan(rank, cfg):
@@ -198,25 +214,166 @@ def job_value(world, calls_per_step, n_bonds, ms_per_step):
 
 
 def run_reference(args):
-    """--impl reference: the oracle timed on the host cores (this tier has no other reference implementation)."""
+    """--impl reference: the oracle timed on the host cores (this tier has no other reference implementation), on the
+    configured workload itself, generated by the oracle's own CPU generators."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     n, m, text = describe(args.workload)
-    steps, warmup = max(1, args.steps), max(0, args.warmup)
-    # keep the whole run within a few minutes: a 2^22-site sweep costs about 2 s per step
-    steps_eff, warmup_eff = min(steps, 20), min(warmup, 3)
-    value, per_step, sample = cpu_oracle_sample(args.workload, steps_eff, warmup_eff)
+    ps = WORKLOADS[args.workload][3]
+    no, src, dst, masks, what = oracle_inputs(args.workload)
+    value, per_step, steps, warmup = time_oracle(args.workload, no, src, dst, masks, max(1, args.steps), max(0, min(args.warmup, 1)),
+                                                 CPU_BUDGET_S)
+    sample = what + ", p sweep " + ",".join("%.4g" % p for p in ps) + ", the configured graph and seeds; labeling time only, 1 thread"
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": "Gbonds/s", "n_gpus": args.gpus,
-        "steps": steps_eff, "warmup": warmup_eff, "ms_per_step": per_step * 1e3, "higher_is_better": True,
+        "steps": steps, "warmup": warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-        "config": {"workload": text, "sample": sample},
-        "cpu_baseline": {"value": value, "unit": "Gbonds/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "config": {"workload": text, "calls_per_step": len(masks), "api": "oracle_label_bits (oracle/ccl_oracle.c)",
+                   "steps_note": "steps cut to fit %.0f s of CPU labeling; the graph is never reduced" % CPU_BUDGET_S},
+        "cpu_baseline": {"value": value, "unit": "Gbonds/s", "cores": 1, "kind": "oracle", "sample": sample,
+                         "host_cores_available": os.cpu_count()},
         "e2e": {"value": value, "unit": "Gbonds/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+class Workload:
+    """A workload resident in HBM: bond list, one occupancy mask per p, a label buffer; generated on the device by the
+    library's own seeded generators (bit-identical to the oracle's: tests/test_gpu_generators_stats.py)."""
+
+    def __init__(self, ccl, torch, name, rank):
+        self.ccl, self.torch, self.name = ccl, torch, name
+        self.fam, self.size, self.z, self.ps, self.kind, self.cfg = WORKLOADS[name]
+        self.n, self.m, self.text = describe(name)
+        fam, size, z, n, m = self.fam, self.size, self.z, self.n, self.m
+        seed = SEED_BASE + self.cfg
+        self.batch = z if fam == "honeycomb_batch" else 1            # realizations labeled per call
+        if fam == "regular":
+            self.src, self.dst = ccl.gen_regular(n, z, seed)
+        elif fam == "cayley":
+            perm = None
+            if z:                                               # "random" numbering (PAPER.md:189): a seeded permutation
+                gen = torch.Generator(device="cuda")
+                gen.manual_seed(seed & 0x7FFFFFFF)
+                perm = torch.randperm(n, device="cuda", generator=gen).to(torch.int32)
+            _, self.src, self.dst = ccl.gen_cayley3(size, perm)
+        elif fam.startswith("honeycomb"):
+            self.src, self.dst = ccl.gen_honeycomb(size)
+        else:
+            self.src, self.dst = ccl.gen_triangular(size)
+        self.masks = []
+        plan = replica_plan(rank, self.cfg)
+        for p in self.ps:                     # replicas differ by realization = rank
+            if self.batch > 1:
+                words = (m + 31) // 32
+                bits = torch.empty((self.batch, words), dtype=torch.int32, device="cuda")
+                for r in range(self.batch):
+                    bits[r] = ccl.gen_occupancy(m, p, plan["seed"], plan["realization"] * self.batch + r, want_mask=False)[1]
+                self.masks.append(bits)
+                continue
+            mask, bits = ccl.gen_occupancy(m, p, plan["seed"], plan["realization"], want_mask=(self.kind == "u8"),
+                                           want_bits=(self.kind != "u8"))
+            self.masks.append(mask if self.kind == "u8" else bits)
+        self.nn_lists = []
+        if fam == "triangular_nn":          # NN list of the occupied bonds, every bond at both ends, built with torch ops (untimed)
+            for bits in self.masks:
+                b = torch.arange(m, device="cuda")
+                on = ((bits[b >> 5] >> (b & 31)) & 1).bool()
+                u, v = self.src[on].long(), self.dst[on].long()
+                a, c = torch.cat([u, v]), torch.cat([v, u])
+                a, order = torch.sort(a, stable=True)
+                c = c[order]
+                deg = torch.bincount(a, minlength=n)
+                start = torch.cumsum(deg, 0) - deg
+                slot = torch.arange(a.numel(), device="cuda") - start[a]
+                nn = torch.full((int(deg.max().item()), n), -1, dtype=torch.int32, device="cuda")
+                nn[slot, a] = c.to(torch.int32)
+                self.nn_lists.append(nn)
+                del b, on, u, v, a, c, order, deg, start, slot
+        self.labels = torch.empty(n * self.batch, dtype=torch.int32, device="cuda")
+        self.api = ("ccl_label_nn" if self.nn_lists else "ccl_label_batch" if self.batch > 1 else
+                    "ccl_label" if self.kind == "u8" else "ccl_label_bits")
+        self.stream_bytes = 8 * m + (m if self.kind == "u8" else 4 * ((m + 31) // 32))
+        self.call_bytes = min_bytes(n, m, self.kind)
+        if self.batch > 1:       # per call: the bond list once, a mask and 12 N of label traffic per realization
+            self.stream_bytes = self.call_bytes = 8 * m + self.batch * (4 * ((m + 31) // 32) + 12 * n)
+        if self.nn_lists:        # the NN list is read twice (steps (i) and (iii)) + 12 N of label traffic
+            self.stream_bytes = self.call_bytes = 2 * 4 * self.nn_lists[0].numel() + 12 * n
+        # L2 hygiene: the bond stream of cfg2-5 (0.2-1.1 GB) exceeds the 126 MB L2, so every call streams from HBM; for
+        # the small cfg1 an L2-sized buffer is rewritten between timed calls.
+        self.flush = None
+        if self.call_bytes < 512 * 1024 * 1024:
+            self.flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+
+    def one_call(self, k):
+        ccl, n = self.ccl, self.n
+        if self.nn_lists:
+            ccl.label_nn(self.nn_lists[k], labels=self.labels)
+        elif self.batch > 1:
+            ccl.label_batch(n, self.src, self.dst, self.masks[k], self.batch, labels=self.labels.view(self.batch, n))
+        elif self.kind == "u8":
+            ccl.label(n, self.src, self.dst, self.masks[k], labels=self.labels)
+        else:
+            ccl.label_bits(n, self.src, self.dst, self.masks[k], labels=self.labels)
+
+    def measure(self, K, warmup, barrier, kernel_split=True):
+        """W warm-up steps, then K timed steps (one call per p each), CUDA events on the launching stream.  Returns the
+        per-call times and the per-step split the library records between its kernels."""
+        torch, ccl, ps = self.torch, self.ccl, self.ps
+        for _ in range(max(3, warmup)):
+            for k in range(len(ps)):
+                self.one_call(k)
+        barrier()
+        ncalls = K * len(ps)
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(ncalls)]
+        split = kernel_split and self.batch == 1 and not self.nn_lists
+        launches0 = ccl.launch_count()
+        barrier()
+        t_start = torch.cuda.Event(enable_timing=True)
+        t_stop = torch.cuda.Event(enable_timing=True)
+        t_start.record()
+        c = 0
+        for _ in range(K):
+            for k in range(len(ps)):
+                if self.flush is not None:
+                    self.flush.fill_(c & 0xFF)
+                e = ev[c]
+                if not split:                                   # no per-step events inside the call
+                    e[0].record(); e[1].record()
+                    self.one_call(k)
+                    e[2].record(); e[3].record()
+                else:
+                    ccl.set_profile_events(e[1], e[2], e[3])
+                    e[0].record()
+                    self.one_call(k)
+                c += 1
+        t_stop.record()
+        barrier()
+        launches = ccl.launch_count() - launches0
+        ccl.set_profile_events(None, None, None)
+        total_ms = t_start.elapsed_time(t_stop)
+        call_ms = [e[0].elapsed_time(e[3]) for e in ev]
+        if self.flush is not None:
+            total_ms = sum(call_ms)                       # exclude the flush writes from the step time
+        return {"total_ms": total_ms, "call_ms": call_ms, "init_ms": [e[0].elapsed_time(e[1]) for e in ev],
+                "reduce_ms": [e[1].elapsed_time(e[2]) for e in ev], "flat_ms": [e[2].elapsed_time(e[3]) for e in ev],
+                "launches": launches, "ncalls": ncalls}
+
+    def per_p(self, r, peak):
+        avg = lambda xs: sum(xs) / len(xs)
+        out = {}
+        n, m, batch = self.n, self.m, self.batch
+        for k, p in enumerate(self.ps):
+            sel = [i for i in range(r["ncalls"]) if i % len(self.ps) == k]
+            t = avg([r["call_ms"][i] for i in sel])
+            out["%.4g" % p] = {"ms": t, "init_ms": avg([r["init_ms"][i] for i in sel]),
+                               "reduce_ms": avg([r["reduce_ms"][i] for i in sel]), "flatten_ms": avg([r["flat_ms"][i] for i in sel]),
+                               "gbonds_per_s": m * batch / (t * 1e-3) / 1e9, "gsites_per_s": n * batch / (t * 1e-3) / 1e9,
+                               "roofline_frac_measured": self.call_bytes / (t * 1e-3) / 1e9 / peak,
+                               "roofline_frac_8TBs": self.call_bytes / (t * 1e-3) / 1e9 / 8000.0}
+        return out
 
 
 def run_ours(args):
@@ -234,138 +391,34 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    fam, size, z, ps, kind, cfg = WORKLOADS[args.workload]
-    n, m, text = describe(args.workload)
-    seed = SEED_BASE + cfg
     if args.region_shift >= 0 or args.force_mode >= 0:
         ccl.set_tuning(-1, args.region_shift, args.force_mode)
     for kv in args.option:
         k, v = kv.split("=")
         ccl.set_option(k, int(v))
-    # ---- synthetic inputs, generated on the device by the library's own seeded generators (untimed)
-    batch = z if fam == "honeycomb_batch" else 1            # realizations labeled per call
-    if fam == "regular":
-        src, dst = ccl.gen_regular(n, z, seed)
-    elif fam == "cayley":
-        perm = None
-        if z:                                               # "random" numbering: a seeded permutation
-            gen = torch.Generator(device="cuda")
-            gen.manual_seed(seed & 0x7FFFFFFF)
-            perm = torch.randperm(n, device="cuda", generator=gen).to(torch.int32)
-        _, src, dst = ccl.gen_cayley3(size, perm)
-    elif fam.startswith("honeycomb"):
-        src, dst = ccl.gen_honeycomb(size)
-    else:
-        src, dst = ccl.gen_triangular(size)
-    masks = []
-    plan = replica_plan(rank, cfg)
-    for p in ps:                      # replicas differ by realization = rank
-        if batch > 1:
-            words = (m + 31) // 32
-            bits = torch.empty((batch, words), dtype=torch.int32, device="cuda")
-            for r in range(batch):
-                bits[r] = ccl.gen_occupancy(m, p, plan["seed"], plan["realization"] * batch + r, want_mask=False)[1]
-            masks.append(bits)
-            continue
-        mask, bits = ccl.gen_occupancy(m, p, plan["seed"], plan["realization"], want_mask=(kind == "u8"),
-                                       want_bits=(kind != "u8"))
-        masks.append(mask if kind == "u8" else bits)
-    nn_lists = []
-    if fam == "triangular_nn":          # NN list of the occupied bonds, every bond at both ends, built with torch ops (untimed)
-        for bits in masks:
-            b = torch.arange(m, device="cuda")
-            on = ((bits[b >> 5] >> (b & 31)) & 1).bool()
-            u, v = src[on].long(), dst[on].long()
-            a, c = torch.cat([u, v]), torch.cat([v, u])
-            a, order = torch.sort(a, stable=True)
-            c = c[order]
-            deg = torch.bincount(a, minlength=n)
-            start = torch.cumsum(deg, 0) - deg
-            slot = torch.arange(a.numel(), device="cuda") - start[a]
-            nn = torch.full((int(deg.max().item()), n), -1, dtype=torch.int32, device="cuda")
-            nn[slot, a] = c.to(torch.int32)
-            nn_lists.append(nn)
-            del b, on, u, v, a, c, order, deg, start, slot
-    labels = torch.empty(n * batch, dtype=torch.int32, device="cuda")
-    torch.cuda.synchronize()
-    torch.cuda.empty_cache()
-
-    def one_call(k):
-        if nn_lists:
-            ccl.label_nn(nn_lists[k], labels=labels)
-        elif batch > 1:
-            ccl.label_batch(n, src, dst, masks[k], batch, labels=labels.view(batch, n))
-        elif kind == "u8":
-            ccl.label(n, src, dst, masks[k], labels=labels)
-        else:
-            ccl.label_bits(n, src, dst, masks[k], labels=labels)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # L2 hygiene: the bond stream of cfg2-5 (0.2-1.1 GB) exceeds the 126 MB L2, so every call streams from HBM; for
-    # the small cfg1 an L2-sized buffer is rewritten between timed calls.
-    flush = None
-    if min_bytes(n, m, kind) < 512 * 1024 * 1024:
-        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
-
-    for _ in range(max(3, args.warmup)):
-        for k in range(len(ps)):
-            one_call(k)
-    barrier()
-
-    K = max(1, args.steps)
-    ncalls = K * len(ps)
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(ncalls)]
-    sampler = ClockSampler(local)
-    sampler.start()
-    launches0 = ccl.launch_count()
-    barrier()
-    t_start = torch.cuda.Event(enable_timing=True)
-    t_stop = torch.cuda.Event(enable_timing=True)
-    flush_ms = 0.0
-    t_start.record()
-    c = 0
-    for _ in range(K):
-        for k in range(len(ps)):
-            if flush is not None:
-                flush.fill_(c & 0xFF)
-            e = ev[c]
-            if batch > 1 or nn_lists or args.no_kernel_split:   # no per-step events inside the call
-                e[0].record(); e[1].record()
-                one_call(k)
-                e[2].record(); e[3].record()
-            else:
-                ccl.set_profile_events(e[1], e[2], e[3])
-                e[0].record()
-                one_call(k)
-            c += 1
-    t_stop.record()
-    barrier()
-    launches = ccl.launch_count() - launches0
-    clocks = sampler.stop()
-    ccl.set_profile_events(None, None, None)
-    total_ms = t_start.elapsed_time(t_stop)
-    call_ms = [e[0].elapsed_time(e[3]) for e in ev]
-    init_ms = [e[0].elapsed_time(e[1]) for e in ev]
-    reduce_ms = [e[1].elapsed_time(e[2]) for e in ev]
-    flat_ms = [e[2].elapsed_time(e[3]) for e in ev]
-    if flush is not None:
-        total_ms = sum(call_ms)                       # exclude the flush writes from the step time
-    total_ms = max_over_ranks(total_ms, world, "cuda")
-    ms_per_step = total_ms / K
-    value = job_value(world, len(ps), m * batch, ms_per_step)
-
     peak, peak_src = measured_peak()
     avg = lambda xs: sum(xs) / len(xs)
-    stream_bytes = 8 * m + (m if kind == "u8" else 4 * ((m + 31) // 32))
-    call_bytes = min_bytes(n, m, kind)
-    if batch > 1:            # per call: the bond list once, a mask and 12 N of label traffic per realization
-        stream_bytes = call_bytes = 8 * m + batch * (4 * ((m + 31) // 32) + 12 * n)
-    if nn_lists:             # the NN list is read twice (steps (i) and (iii)) + 12 N of label traffic
-        stream_bytes = call_bytes = 2 * 4 * nn_lists[0].numel() + 12 * n
+    w = Workload(ccl, torch, args.workload, rank)
+    n, m, ps, kind, batch, fam, size = w.n, w.m, w.ps, w.kind, w.batch, w.fam, w.size
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+
+    K = max(1, args.steps)
+    sampler = ClockSampler(local)
+    sampler.start()
+    r = w.measure(K, args.warmup, barrier, kernel_split=not args.no_kernel_split)
+    clocks = sampler.stop()
+    total_ms = max_over_ranks(r["total_ms"], world, "cuda")
+    ms_per_step = total_ms / K
+    value = job_value(world, len(ps), m * batch, ms_per_step)
+    call_ms, init_ms, reduce_ms, flat_ms, launches = r["call_ms"], r["init_ms"], r["reduce_ms"], r["flat_ms"], r["launches"]
+    stream_bytes, call_bytes = w.stream_bytes, w.call_bytes
     ach = stream_bytes / (avg(reduce_ms) * 1e-3) / 1e9
     traffic = None
     try:
@@ -374,21 +427,13 @@ def run_ours(args):
     except Exception:
         pass
     call_ach = call_bytes / (avg(call_ms) * 1e-3) / 1e9
-    per_p = {}
-    for k, p in enumerate(ps):
-        sel = [i for i in range(ncalls) if i % len(ps) == k]
-        t = avg([call_ms[i] for i in sel])
-        per_p["%.4g" % p] = {"ms": t, "init_ms": avg([init_ms[i] for i in sel]),
-                             "reduce_ms": avg([reduce_ms[i] for i in sel]), "flatten_ms": avg([flat_ms[i] for i in sel]),
-                             "gbonds_per_s": m * batch / (t * 1e-3) / 1e9, "gsites_per_s": n * batch / (t * 1e-3) / 1e9,
-                             "roofline_frac_measured": call_bytes / (t * 1e-3) / 1e9 / peak,
-                             "roofline_frac_8TBs": call_bytes / (t * 1e-3) / 1e9 / 8000.0}
+    per_p = w.per_p(r, peak)
 
     # ---- end to end through the host-buffer entry point: H2D of the inputs and D2H of the labels inside the timing
     e2e = None
-    if not args.no_e2e and kind != "u8" and batch == 1 and not nn_lists:
-        hs, hd = src.cpu().pin_memory(), dst.cpu().pin_memory()
-        hm = [b.cpu().pin_memory() for b in masks]
+    if not args.no_e2e and kind != "u8" and batch == 1 and not w.nn_lists:
+        hs, hd = w.src.cpu().pin_memory(), w.dst.cpu().pin_memory()
+        hm = [b.cpu().pin_memory() for b in w.masks]
         hl = torch.empty(n, dtype=torch.int32).pin_memory()
         # the call a user makes for an occupancy sweep: ccl_label_sweep_host (bond list uploaded once, labels of mask k
         # travel back while mask k+1 is labeled); a single p goes through ccl_label_bits_host
@@ -417,19 +462,20 @@ def run_ours(args):
                        if sweep else "ccl_label_bits_host (pinned host src/dst/bits in, host labels out, synchronous)")}
         del hls
         del hs, hd, hm, hl
+        ccl.trim_scratch(0)                                           # the host-buffer calls' device copies go back to the driver
 
     # ---- config 3 asks for "largest-cluster and wrapping statistics per p": untimed, after the timed region
     statistics = None
-    if rank == 0 and fam in ("triangular", "honeycomb") and kind != "u8" and not nn_lists:
+    if rank == 0 and fam in ("triangular", "honeycomb") and kind != "u8" and not w.nn_lists:
         statistics = {}
         wx, wy = ccl.gen_wrap_vectors(fam, size)
         for k, p in enumerate(ps):
             t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True); t2 = torch.cuda.Event(enable_timing=True)
-            one_call(k)
+            w.one_call(k)
             t0.record()
-            st, _, _ = ccl.cluster_stats(labels, 0)
+            st, _, _ = ccl.cluster_stats(w.labels, 0)
             t1.record()
-            wrap_x, wrap_y, _ = ccl.wrap(n, src, dst, masks[k], wx, wy)
+            wrap_x, wrap_y, _ = ccl.wrap(n, w.src, w.dst, w.masks[k], wx, wy)
             t2.record()
             torch.cuda.synchronize()
             statistics["%.4g" % p] = {"n_clusters": st["n_clusters"], "largest": st["largest"], "largest_over_n": st["largest"] / n,
@@ -437,23 +483,61 @@ def run_ours(args):
                                       "wrap_ms_incl_open_labeling": t1.elapsed_time(t2)}
         del wx, wy
 
+    # ---- the oracle, one thread, on the very same graph and masks (downloaded: the device generators are bit-identical
+    #      to the oracle's), timed in the same run on this host's cores
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
-        v, per_step, sample = cpu_oracle_sample(args.workload, 3, 1)
-        cpu = {"value": v, "unit": "Gbonds/s", "cores": 1, "kind": "oracle", "sample": sample,
-               "host_cores_available": os.cpu_count()}
+        import numpy as np
+        reps = min(batch, 64)
+        hsrc, hdst = w.src.cpu().numpy(), w.dst.cpu().numpy()
+        if batch > 1:
+            hmasks = [(None, np.ascontiguousarray(b[j].cpu().numpy().view(np.uint32))) for b in w.masks for j in range(reps)]
+        elif kind == "u8":
+            hmasks = [(b.cpu().numpy(), None) for b in w.masks]
+        else:
+            hmasks = [(None, np.ascontiguousarray(b.cpu().numpy().view(np.uint32))) for b in w.masks]
+        v, per_step, steps_cpu, _ = time_oracle(args.workload, n, hsrc, hdst, hmasks, 1 if per_p and avg(call_ms) > 0.3 else 3,
+                                                0 if n >= (1 << 22) else 1, 60.0)
+        cpu = {"value": v, "unit": "Gbonds/s", "cores": 1, "kind": "oracle", "host_cores_available": os.cpu_count(),
+               "seconds_per_step": per_step, "steps": steps_cpu,
+               "sample": "the benchmarked workload itself (%s; same graph, same masks, downloaded from the device)%s; "
+                         "labeling time only (oracle_label%s), 1 thread" % (
+                             w.text, " limited to %d realizations per p" % reps if batch > 1 else "", "" if kind == "u8" else "_bits")}
+        del hsrc, hdst, hmasks
+
+    # ---- the other BASELINE.json configs, a few steps each, same timing (north_star: "report throughput on the five configs")
+    configs = None
+    if rank == 0 and args.workload == "cfg5" and not args.no_other_configs:
+        configs = {}
+        del w
+        torch.cuda.empty_cache()
+        for name in ("cfg1", "cfg2", "cfg3", "cfg4"):
+            wk = Workload(ccl, torch, name, rank)
+            torch.cuda.synchronize()
+            rr = wk.measure(5, 3, lambda: torch.cuda.synchronize())
+            t = avg(rr["call_ms"])
+            configs[name] = {"workload": wk.text, "api": wk.api, "ms_per_call": t, "steps": 5, "warmup": 3,
+                             "gbonds_per_s": wk.m / (t * 1e-3) / 1e9, "gsites_per_s": wk.n / (t * 1e-3) / 1e9,
+                             "bytes_per_call": wk.call_bytes,
+                             "roofline_call_frac": wk.call_bytes / (t * 1e-3) / 1e9 / peak,
+                             "roofline_call_frac_8TBs": wk.call_bytes / (t * 1e-3) / 1e9 / 8000.0,
+                             "gpu_launches_per_call": rr["launches"] / rr["ncalls"], "per_p": wk.per_p(rr, peak),
+                             "l2": "256 MB buffer rewritten between timed calls" if wk.flush is not None else "inputs larger than L2"}
+            del wk
+            torch.cuda.empty_cache()
 
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": "Gbonds/s", "n_gpus": world, "steps": K,
             "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": text, "calls_per_step": len(ps), "api": "ccl_label_nn" if nn_lists else "ccl_label_batch" if batch > 1 else "ccl_label" if kind == "u8" else "ccl_label_bits",
+            "config": {"workload": describe(args.workload)[2], "calls_per_step": len(ps),
+                       "api": "ccl_label_nn" if fam == "triangular_nn" else "ccl_label_batch" if batch > 1 else "ccl_label" if kind == "u8" else "ccl_label_bits",
                        "parallelism": "replicas x%d (one realization per GPU, no collective)" % world,
                        "l2": "inputs larger than L2 (bond stream %.0f MB per call vs 126 MB L2)" % (stream_bytes / 1e6)
-                       if flush is None else "256 MB buffer rewritten between timed calls (L2 flush)",
+                       if call_bytes >= 512 * 1024 * 1024 else "256 MB buffer rewritten between timed calls (L2 flush)",
                        "gsites_per_s": world * len(ps) * n * batch / (ms_per_step * 1e-3) / 1e9},
-            "roofline": {"bound": "hbm", "kernel": "k_label_batch (steps i-iv)" if batch > 1 else "step (iii): k_reduce, or k_scatter + k_descend x regions", "achieved": ach, "peak": peak, "unit": "GB/s",
+            "roofline": {"bound": "hbm", "kernel": "k_label_batch (steps i-iv)" if batch > 1 else "step (iii): k_reduce / k_hook + k_join, or k_scatter_tiles + k_descend x regions", "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": stream_bytes, "avg_launch_ms": avg(reduce_ms),
                          "share_of_call": avg(reduce_ms) / avg(call_ms)},
@@ -461,13 +545,13 @@ def run_ours(args):
                               "achieved": call_ach, "peak": peak, "unit": "GB/s", "frac": call_ach / peak,
                               "frac_of_8TBs_nominal": call_ach / 8000.0, "bytes_per_call": call_bytes,
                               "avg_call_ms": avg(call_ms)},
-            "roofline_kernels": None if (batch > 1 or nn_lists) else {
-                "k_init (step i)": {"algorithmic_bytes": 4 * n, "avg_ms": avg(init_ms),
-                                    "frac": 4 * n / (avg(init_ms) * 1e-3) / 1e9 / peak},
+            "roofline_kernels": None if (batch > 1 or fam == "triangular_nn") else {
+                "step (i) where it is a pass of its own": {"algorithmic_bytes": 4 * n, "avg_ms": avg(init_ms)},
                 "step (iii)": {"algorithmic_bytes": stream_bytes, "avg_ms": avg(reduce_ms), "frac": ach / peak},
                 "k_flatten (step iv)": {"algorithmic_bytes": 8 * n, "avg_ms": avg(flat_ms),
                                         "frac": 8 * n / (avg(flat_ms) * 1e-3) / 1e9 / peak}},
             "per_p": per_p, "kernel_ms": {"k_init": avg(init_ms), "k_reduce": avg(reduce_ms), "k_flatten": avg(flat_ms)},
+            "configs": configs,
             "statistics": statistics, "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
         }
         print(json.dumps(line), flush=True)
@@ -497,6 +581,7 @@ def main():
                     help="do not record events between the kernels of a call (an event record between two kernels keeps them "
                          "from overlapping by programmatic dependent launch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="cfg5 only: do not also measure cfg1-cfg4 afterwards")
     args = ap.parse_args()
     if args.family:
         ps = [float(t) for t in args.p.split(",") if t]

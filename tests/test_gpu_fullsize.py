@@ -50,6 +50,34 @@ def test_cfg3_honeycomb_L4096(ccl):
     _check(ccl, 2 * L * L, src, dst, d_src, d_dst, [0.60, 0.6527, 0.70], 3)
 
 
+def test_cfg3_wrapping_statistics_L4096(ccl):
+    """Config 3 asks for wrapping statistics per p, and the crossing of the wrapping probability at p_c is the paper's own
+    correctness evidence.  ccl_wrap (open-lattice labels, a 128 MiB label array, + seam-graph union-find)
+    against the oracle's displacement union-find at the full size, for the three configured p and three realizations at
+    the threshold itself, where the answer is not a foregone conclusion."""
+    L = 4096
+    n = 2 * L * L
+    src, dst, dx, dy = oracle.gen_honeycomb(L, with_disp=True)
+    cell = src.astype(np.int64) // 2
+    wx = ((cell % L + dx) // L).astype(np.int8)
+    wy = ((cell // L + dy) // L).astype(np.int8)
+    d_src, d_dst = ccl.gen_honeycomb(L)
+    gx, gy = ccl.gen_wrap_vectors("honeycomb", L)
+    assert np.array_equal(gx.cpu().numpy(), wx) and np.array_equal(gy.cpu().numpy(), wy)
+    seen = set()
+    for p, r in [(0.60, 0), (0.6527, 0), (0.70, 0), (0.6527, 1), (0.6527, 2), (0.6527, 3)]:
+        mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(3), r)
+        want = oracle.wrap(n, src, dst, dx, dy, mask)
+        got_x, got_y, lab_open = ccl.wrap(n, d_src, d_dst, torch.from_numpy(bits.view(np.int32)).cuda(), gx, gy)
+        assert (got_x, got_y) == want, (p, r)
+        seen.add(want)
+        if r == 0:
+            open_mask = mask & ((wx == 0) & (wy == 0)).astype(np.uint8)
+            assert np.array_equal(lab_open.cpu().numpy(), oracle.label(n, src, dst, open_mask)), p
+        del mask, bits, lab_open
+    assert (False, False) in seen and (True, True) in seen
+
+
 def test_cfg4_regular3_2p24(ccl):
     n = 1 << 24
     src, dst, _ = oracle.gen_regular(n, 3, oracle.seed_for(4))

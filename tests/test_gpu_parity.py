@@ -318,6 +318,91 @@ def test_two_pass_form(options, two_pass):
         assert all_zero(ccl.label(n, dev(src), dev(dst)))
 
 
+def test_options_belong_to_the_calling_thread(ccl):
+    """ccl_set_option on another host thread cannot change a call on this one (and vice versa): the knobs are
+    thread-local like the error string and the launch counter, and a call reads them once on entry."""
+    import threading
+    rng = np.random.default_rng(77)
+    n, m = 50000, 120000
+    src, dst = graphs.random_graph(rng, n, m)
+    s, d = dev(src), dev(dst)
+    want = oracle.label(n, src, dst)
+    ccl.set_option("reset")
+    base = ccl.launch_count()
+    ccl.label(n, s, d)
+    plain = ccl.launch_count() - base                      # direct form: k_init, k_reduce, k_flatten
+    seen = {}
+
+    def other():
+        torch.cuda.set_device(0)
+        ccl.set_option("bucket_min_label_bytes", 0)        # on THIS thread every call takes the bucketed form
+        ccl.set_option("region_shift", 12)
+        ccl.set_option("force_mode", 1)
+        before = ccl.launch_count()
+        got = ccl.label(n, s, d)
+        seen["launches"] = ccl.launch_count() - before
+        seen["ok"] = bool(np.array_equal(got.cpu().numpy(), want))
+    t = threading.Thread(target=other)
+    t.start()
+    t.join()
+    assert seen["ok"] and seen["launches"] > plain         # the other thread really ran another path
+    base = ccl.launch_count()
+    got = ccl.label(n, s, d)
+    assert ccl.launch_count() - base == plain              # ... and this thread's options are untouched
+    assert np.array_equal(got.cpu().numpy(), want)
+
+
+def test_scratch_is_reported_and_can_be_trimmed(ccl):
+    """include/ccl.h: scratch stays in the library's pool for the next call until ccl_trim_scratch hands it back."""
+    torch.cuda.synchronize()
+    ccl.trim_scratch(0)                                    # whatever earlier tests left in the pool
+    ccl.set_tuning(0, 16, 1, 0)                            # bucketed form: draws a workspace
+    rng = np.random.default_rng(5)
+    n, m = 1 << 20, 1 << 22                                # cfg4-like shape, scaled
+    src, dst = graphs.random_graph(rng, n, m)
+    got = ccl.label(n, dev(src), dev(dst))
+    torch.cuda.synchronize()
+    reserved, in_use = ccl.scratch_bytes()
+    assert reserved >= 8 * m and in_use == 0               # pair chunks for >= m pairs were drawn and returned to the pool
+    assert reserved <= 16 * m + (64 << 20)                 # ... and the pool is sized by the pairs that can exist (1.25 M), not 4 M
+    ccl.trim_scratch(0)
+    assert ccl.scratch_bytes()[0] == 0
+    assert np.array_equal(got.cpu().numpy(), oracle.label(n, src, dst))
+    assert np.array_equal(ccl.label(n, dev(src), dev(dst)).cpu().numpy(), got.cpu().numpy())     # works again after a trim
+    ccl.set_tuning()
+    ccl.trim_scratch(0)
+
+
+def test_probe_cache_on_and_off(ccl):
+    """The host-side memory of the device probe's answer changes which kernels are enqueued, never the labels: repeated
+    calls on one bond list (first call: probe undecided, later calls: decided) and the same with the cache off."""
+    rng = np.random.default_rng(21)
+    n, m = 200000, 500000
+    for local in (False, True):
+        src, dst = graphs.random_graph(rng, n, m)
+        if local:
+            dst = np.clip(src + rng.integers(-3, 4, size=m), 0, n - 1).astype(np.int32)
+        s, d = dev(src), dev(dst)
+        for cache in (1, 0):
+            ccl.set_option("reset")
+            ccl.set_option("bucket_min_label_bytes", 0)
+            ccl.set_option("region_shift", 13)
+            ccl.set_option("probe_cache", cache)
+            counts = []
+            for rep in range(4):
+                mask = (rng.random(m) < 0.6).astype(np.uint8)
+                before = ccl.launch_count()
+                got = ccl.label(n, s, d, dev(mask))
+                torch.cuda.synchronize()                   # lets the probe's answer reach the host
+                counts.append(ccl.launch_count() - before)
+                assert np.array_equal(got.cpu().numpy(), oracle.label(n, src, dst, mask)), (local, cache, rep)
+            if cache and local:
+                assert counts[-1] < counts[0]              # once decided, only the chosen (direct) form is enqueued
+            elif not cache:
+                assert counts[-1] == counts[0]
+    ccl.set_option("reset")
+
+
 def test_tuning_argument_checks(ccl):
     with pytest.raises(ccl.CclError):
         ccl.set_tuning(0, 2, 0)
