@@ -96,6 +96,7 @@ extern "C" int ccl_set_option(const char* name, int64_t value)
     }
     if (!strcmp(name, "bucket_capacity")) { t.bucket_capacity = value > 0 ? value : 0; return CCL_OK; }
     if (!strcmp(name, "two_pass")) { t.two_pass = value > 0 ? 1 : value < 0 ? -1 : 0; return CCL_OK; }
+    if (!strcmp(name, "warp_premerge")) { t.warp_premerge = value != 0; return CCL_OK; }
     if (!strcmp(name, "scatter_tiles")) { t.scatter_tiles = value != 0; return CCL_OK; }
     if (!strcmp(name, "probe_cache")) { t.probe_cache = value != 0; return CCL_OK; }
     if (!strcmp(name, "flatten_window_bytes")) {

@@ -237,8 +237,8 @@ k_scatter_tiles(int64_t n_tiles, const int32_t* __restrict__ src, const int32_t*
 // -------------------------------------------------------------------------------------------------- descend
 // Reduce region r: all label[] traffic of this launch falls into [r << shift, (r+1) << shift).  init_lo < init_hi: the
 // labels of the region that comes next are written on the way out (step (i) for that region).
-__global__ void __launch_bounds__(kBThreads, 6)
-k_descend(int r, BucketRef bk, int gated, int64_t init_lo, int64_t init_hi, int32_t* label)
+__global__ void __launch_bounds__(kBThreads, 8)
+k_descend(int r, BucketRef bk, int gated, int64_t init_lo, int64_t init_hi, int premerge, int32_t* label)
 {
     constexpr int P = kDescendP;
     __shared__ EmitSmem sm;
@@ -299,12 +299,32 @@ k_descend(int r, BucketRef bk, int gated, int64_t init_lo, int64_t init_hi, int3
                     else v[k] = label[nb];
                 }
             }
+            if (premerge) {
+                // Experiment (ccl_set_option "warp_premerge", off by default; profiles/r2_premerge.md): lanes whose
+                // atomics target the same site b elect the smallest partner; one lane links b to it, the others go on
+                // with {a_min, a} as if they had read label[b] = a_min.
+                const int lane = threadIdx.x & 31;
 #pragma unroll
-            for (int k = 0; k < P; ++k)
-                if (act[k]) old[k] = (v[k] > a[k]) ? atomicMin(label + b[k], a[k]) : v[k];
+                for (int k = 0; k < P; ++k) {
+                    const bool need = act[k] && v[k] > a[k];
+                    const unsigned peers = __match_any_sync(0xffffffffu, need ? b[k] : ~lane);
+                    const int32_t amin = __reduce_min_sync(peers, a[k]);
+                    const unsigned mins = __ballot_sync(0xffffffffu, a[k] == amin) & peers;
+                    if (act[k]) {
+                        if (!need) old[k] = v[k];
+                        else if (lane == __ffs(mins) - 1) old[k] = atomicMin(label + b[k], a[k]);
+                        else old[k] = amin;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < P; ++k)
+                    if (act[k]) old[k] = (v[k] > a[k]) ? atomicMin(label + b[k], a[k]) : v[k];
+            }
 #pragma unroll
             for (int k = 0; k < P; ++k)
                 if (act[k]) { act[k] = old[k] != b[k] && old[k] != a[k]; any |= act[k]; }
+            if (premerge) any = __any_sync(0xffffffffu, any);          // the pre-merge needs the whole warp in step
             if (!any) break;
         }
         bool pending = false;
@@ -378,6 +398,7 @@ int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, cudaStream
     plan->cshift = cshift;
     plan->n_regions = n_regions;
     plan->scatter_tiles = t.scatter_tiles;
+    plan->premerge = t.warp_premerge;
     CCL_CUDA_TRY(cudaMemsetAsync(ws, 0, hdr_bytes + table_bytes, st));
     return CCL_OK;
 }
@@ -435,7 +456,7 @@ int bucketed_launch(const BucketPlan& plan, int64_t n_sites, int64_t n_bonds, co
             init_hi = (int64_t)r << shift;
             if (init_hi > n_sites) init_hi = n_sites;
         }
-        CCL_CUDA_TRY(launch_pdl(k_descend, (unsigned)grids.descend, (unsigned)kBThreads, st, r, bk, gated, init_lo, init_hi, labels));
+        CCL_CUDA_TRY(launch_pdl(k_descend, (unsigned)grids.descend, (unsigned)kBThreads, st, r, bk, gated, init_lo, init_hi, plan.premerge, labels));
         count_launch();
     }
     return CCL_OK;

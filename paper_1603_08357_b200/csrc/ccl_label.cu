@@ -42,12 +42,13 @@ __device__ __forceinline__ bool gate_open(const BucketHeader* hdr, int kind)
 template <int MASK, bool VEC>
 __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_t* __restrict__ src,
                                        const int32_t* __restrict__ dst, const void* __restrict__ occ,
-                                       int32_t* label, uint64_t pol, int32_t (&pa)[4], int32_t (&pb)[4])
+                                       int32_t* label, uint64_t pol, int premerge, int32_t (&pa)[4], int32_t (&pb)[4])
 {
     // Loads this thread's (up to) 4 bonds, does the first-touch atomics, and returns how many pairs are left to join;
-    // they are stored in pa[]/pb[] front-packed.
-    if (b0 >= n_bonds) return 0;
-    const int cnt = (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
+    // they are stored in pa[]/pb[] front-packed.  (With the pre-merge experiment on, every lane of the warp stays to the
+    // end: the vote needs them all.)
+    if (b0 >= n_bonds && !premerge) return 0;
+    const int cnt = (b0 >= n_bonds) ? 0 : (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
 
     // occupancy of this thread's 4 bonds -> low 4 bits of m
     uint32_t m = 0xFu;
@@ -65,10 +66,11 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
         }
     }
     m &= (1u << cnt) - 1u;
-    if (m == 0) return 0;
+    if (m == 0 && !premerge) return 0;
 
-    int32_t u[4], v[4];
-    if (VEC && cnt == 4) {
+    int32_t u[4] = {0, 0, 0, 0}, v[4] = {0, 0, 0, 0};
+    if (m == 0) {
+    } else if (VEC && cnt == 4) {
         const int4 s = ld_stream_v4(src + b0, pol), d = ld_stream_v4(dst + b0, pol);
         u[0] = s.x; u[1] = s.y; u[2] = s.z; u[3] = s.w;
         v[0] = d.x; v[1] = d.y; v[2] = d.z; v[3] = d.w;
@@ -89,7 +91,19 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
         lo[k] = min(u[k], v[k]);
         const int32_t hi = max(u[k], v[k]);
         old[k] = lo[k];                                    // "nothing left to do"
-        if (((m >> k) & 1u) && hi != lo[k]) {
+        const bool need = ((m >> k) & 1u) && hi != lo[k];
+        if (premerge) {
+            // experiment ("warp_premerge"): bonds of this warp with the same higher site send one atomic, with the smallest
+            // of their lower sites; the others are left with the pair {that site, their own lower site}
+            const int lane = threadIdx.x & 31;
+            const unsigned peers = __match_any_sync(0xffffffffu, need ? hi : ~lane);
+            const int32_t amin = __reduce_min_sync(peers, lo[k]);
+            const unsigned mins = __ballot_sync(0xffffffffu, lo[k] == amin) & peers;
+            if (need) {
+                if (lane == __ffs(mins) - 1) { const int32_t o = atomicMin(label + hi, lo[k]); old[k] = (o == hi) ? lo[k] : o; }
+                else old[k] = amin;                        // == lo[k] for a duplicate: nothing left to do
+            }
+        } else if (need) {
             const int32_t o = atomicMin(label + hi, lo[k]);
             old[k] = (o == hi) ? lo[k] : o;
         }
@@ -112,7 +126,7 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
 template <int MASK, bool VEC>
 __global__ void __launch_bounds__(kThreads)
 k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, int gate)
+         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, int gate, int premerge)
 {
     __shared__ int2 queue[kThreads / 32][128];
     pdl_wait();
@@ -123,7 +137,7 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
     const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
     for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
         int32_t pa[4], pb[4];
-        const int n = reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol, pa, pb);
+        const int n = reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol, premerge, pa, pb);
         int incl = n;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -154,17 +168,28 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
 template <int MASK>
 __global__ void __launch_bounds__(kThreads)
 k_hook(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, const void* __restrict__ occ,
-       int vec, int32_t* label, const BucketHeader* hdr, int gate)
+       int vec, int32_t* label, const BucketHeader* hdr, int gate, int premerge)
 {
     pdl_wait();
     if (!gate_open(hdr, gate)) return;                     // another form did step (iii)
     const uint64_t pol = evict_first_policy();
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
-    for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_bonds; b0 += stride) {
+    const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
+    for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
         const Bonds4 c = load_bonds4<MASK>(n_bonds, b0, src, dst, occ, vec, pol);
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
-            if (((c.m >> k) & 1u) && c.u[k] != c.v[k]) atomicMin(label + max(c.u[k], c.v[k]), min(c.u[k], c.v[k]));
+        for (int k = 0; k < 4; ++k) {
+            const bool need = ((c.m >> k) & 1u) && c.u[k] != c.v[k];
+            const int32_t lo = min(c.u[k], c.v[k]), hi = max(c.u[k], c.v[k]);
+            if (premerge) {                                // experiment ("warp_premerge"): one atomic per distinct higher site
+                const int lane = threadIdx.x & 31;
+                const unsigned peers = __match_any_sync(0xffffffffu, need ? hi : ~lane);
+                const int32_t amin = __reduce_min_sync(peers, lo);
+                if (need && lane == __ffs(peers) - 1) atomicMin(label + hi, amin);
+            } else if (need) {
+                atomicMin(label + hi, lo);
+            }
+        }
     }
 }
 
@@ -336,11 +361,12 @@ static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst
     const int64_t groups = (n_bonds + 3) / 4;
     int64_t blocks = (groups + kThreads - 1) / kThreads;
     if (blocks > (int64_t)kSMs * 8 * 4) blocks = (int64_t)kSMs * 8 * 4;       // grid-stride beyond 4 waves of 8 CTAs/SM
+    const int pm = tuning().warp_premerge;
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     bool vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
-    if (vec) CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, true>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate));
-    else     CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, false>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate));
+    if (vec) CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, true>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, pm));
+    else     CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, false>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, pm));
     count_launch();
     return CCL_OK;
 }
@@ -368,7 +394,7 @@ static int launch_two_pass(int64_t n_sites, int64_t n_bonds, const int32_t* src,
     // hook and the mid-call flatten are this form's own steps (i)/(ii); the join pass also serves as the safety net of
     // the bucketed form (it joins whatever the ends of an occupied bond still differ in)
     const int own = gate == kGateNone ? kGateNone : kGateDirect;
-    CCL_CUDA_TRY(launch_pdl(k_hook<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, own));   // step (i), paper form
+    CCL_CUDA_TRY(launch_pdl(k_hook<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, own, tuning().warp_premerge));   // step (i), paper form
     count_launch();
     { const int rc = launch_flatten(n_sites, labels, 0, n_sites, hdr, own, st); if (rc != CCL_OK) return rc; }                      // step (ii)
     CCL_CUDA_TRY(launch_pdl(k_join<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, gate));   // step (iii)

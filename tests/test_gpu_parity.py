@@ -403,6 +403,36 @@ def test_probe_cache_on_and_off(ccl):
     ccl.set_option("reset")
 
 
+def test_warp_premerge_option(options):
+    """The pre-merge experiment (profiles/r2_premerge.md) changes which lane sends an atomic, never the labels: one-pass,
+    two-pass and bucketed forms, random graphs, lattices (where lanes really share higher sites), stars, duplicates."""
+    ccl = options
+    rng = np.random.default_rng(4711)
+    for extra in ({"two_pass": 0}, {"two_pass": 1}, {"bucket_min_label_bytes": 0, "region_shift": 11, "force_mode": 1}):
+        ccl.set_option("reset")
+        ccl.set_option("warp_premerge", 1)
+        for k, v in extra.items():
+            ccl.set_option(k, v)
+        for trial in range(10):
+            n = int(rng.integers(2, 80000))
+            m = int(rng.integers(1, 4 * n + 1))
+            src, dst = graphs.random_graph(rng, n, m, self_loops=True)
+            if trial % 2:
+                dst = np.clip(src + rng.integers(-2, 3, size=m), 0, n - 1).astype(np.int32)   # many shared higher sites
+            mask = (rng.random(m) < rng.random()).astype(np.uint8)
+            run_all_forms(ccl, n, src, dst, mask)
+        for name in ["honeycomb_L301", "triangular_L257", "regular4"]:
+            n, src, dst, ps, cfg = _case(name)
+            for p in ps + [1.0]:
+                mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(cfg), realization=11)
+                run_all_forms(ccl, n, src, dst, mask)
+        n = 1 << 15
+        hub = np.full(n - 1, n - 1, dtype=np.int32)
+        assert all_zero(ccl.label(n, dev(hub), dev(np.arange(n - 1, dtype=np.int32))))
+        same = np.full(3000, n - 3, dtype=np.int32)        # 3000 copies of one bond
+        assert ccl.label(n, dev(same), dev(np.full(3000, 7, dtype=np.int32))).cpu().numpy()[n - 3] == 7
+
+
 def test_tuning_argument_checks(ccl):
     with pytest.raises(ccl.CclError):
         ccl.set_tuning(0, 2, 0)
