@@ -268,6 +268,36 @@ def test_bucketed_form_workloads_bit_exact(bucketed, name, mode):
         run_all_forms(ccl, n, src, dst, mask)
 
 
+@pytest.mark.parametrize("m", [2047, 2048, 2049, 4096, 6143, 6144 + 7, 10 * 2048 + 2047])
+def test_bucketed_scatter_tile_boundaries(bucketed, m):
+    """The bulk-copy scatter kernel takes whole 2048-bond tiles of 16-byte aligned input, the register kernel the tail,
+    unaligned input and everything when the tiles are switched off: bond counts around the tile size, every mask kind
+    (none, uint8, packed), aligned and unaligned views, both kernels."""
+    ccl = bucketed
+    rng = np.random.default_rng(m)
+    n = 5000
+    src, dst = graphs.random_graph(rng, n, m, self_loops=True)
+    mask = (rng.random(m) < 0.6).astype(np.uint8)
+    want = oracle.label(n, src, dst, mask)
+    want_all = oracle.label(n, src, dst)
+    bits = graphs.pack_bits(mask)
+    for tiles in (1, 0):
+        ccl.set_tuning(0, 9, 1, 0)                     # 2^9-site regions: ten of them
+        ccl.set_option("scatter_tiles", tiles)
+        s, d = dev(src), dev(dst)
+        assert np.array_equal(ccl.label(n, s, d, dev(mask)).cpu().numpy(), want)
+        assert np.array_equal(ccl.label_bits(n, s, d, bits_dev(bits)).cpu().numpy(), want)
+        assert np.array_equal(ccl.label(n, s, d).cpu().numpy(), want_all)
+        # element offset 1: src/dst lose their 16-byte alignment, the masks theirs
+        s1 = dev(np.concatenate([[0], src]).astype(np.int32))[1:]
+        d1 = dev(np.concatenate([[0], dst]).astype(np.int32))[1:]
+        o1 = dev(np.concatenate([[1], mask]).astype(np.uint8))[1:]
+        assert np.array_equal(ccl.label(n, s1, d1, o1).cpu().numpy(), want)
+        assert np.array_equal(ccl.label_bits(n, s1, d1, bits_dev(bits)).cpu().numpy(), want)
+        b1 = dev(np.concatenate([[0], bits.view(np.int32)]).astype(np.int32))[1:]      # packed mask 4-, not 16-byte aligned
+        assert np.array_equal(ccl.label_bits(n, s, d, b1).cpu().numpy(), want)
+
+
 def test_bucketed_form_adversarial(bucketed):
     ccl = bucketed
     ccl.set_tuning(0, 12, 1, 0)
