@@ -1,5 +1,5 @@
 // ccl_bonds.cuh -- streaming load of four consecutive bonds and their occupancy bits, shared by the kernels that read
-// the bond list (ccl_label.cu, ccl_tile.cu).  Product code.
+// the bond list (ccl_label.cu).  Product code.
 #pragma once
 
 #include "ccl_common.cuh"

@@ -216,7 +216,7 @@ __device__ __forceinline__ void probe_regions(const ProbeJob& job)
 // little longer; every decision that matters is re-validated by the value an atomicMin
 // returns.  What L1 buys: the top of a big cluster's tree is read by every walk through that cluster, and with
 // L2-only loads (ld.relaxed.gpu, the first version) those reads all queue up at the one L2 slice that owns the
-// sector (profiles/r1_notes.md).
+// sector (k_flatten on honeycomb p = 0.70: 1.29 ms with L2-only loads, 0.14 ms through L1; round 1).
 __device__ __forceinline__ int32_t ld_label(const int32_t* p)
 {
     int32_t r;
