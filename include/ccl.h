@@ -16,7 +16,8 @@
  *     the call returns.  The pool KEEPS what it has reserved for the next call (so that a sweep of calls does not
  *     pay the driver for memory each time) until ccl_trim_scratch() hands it back; ccl_scratch_bytes() reports it.
  *     What a call draws: ccl_label / ccl_label_bits nothing, unless n_sites * 4 >= 96 MiB and n_bonds >= 2^20 (the
- *     region-bucketed form): then 10 * n_bonds bytes of pair chunks plus a table (about 1.3 GB for 2^27 bonds);
+ *     region-bucketed form): then 10 * n_bonds bytes of pair chunks plus a table (about 1.5 GB for 2^27 bonds; twice,
+ *     four, at most eight times that on a bond list on which an earlier call ran the pool dry);
  *     the host-buffer entry points also their device copies of src, dst, masks and labels.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the default stream).  All work is enqueued on it; no
  *     entry point synchronises with the host unless stated.  Results are valid once the stream has drained.
@@ -202,8 +203,9 @@ int ccl_scratch_bytes(int64_t* reserved, int64_t* in_use);
  *   "region_shift"            a region is 2^value sites (default 23, allowed 4..30; raised automatically so that
  *                             there are at most 32 regions; negative restores the default)
  *   "force_mode"              -1 = the probe decides (default), 0 = always direct, 1 = always bucketed when eligible
- *   "bucket_capacity"         pairs the chunk pool of the bucketed form can hold (<= 0: 1.25 n_bonds + slack); if it
- *                             runs dry the direct kernel re-does the bond list behind the bucketed kernels
+ *   "bucket_capacity"         pairs the chunk pool of the bucketed form can hold (<= 0: 1.25 n_bonds + slack, doubled
+ *                             for later calls on a bond list whenever it ran dry); if it runs dry the direct kernel
+ *                             re-does the bond list behind the bucketed kernels
  *   "scatter_tiles"           1 = the bulk-copy (cp.async.bulk) scatter kernel for 16-byte aligned input (default),
  *                             0 = the register kernel for everything
  *   "probe_cache"             1 = remember the probe's answer per bond list (default), 0 = probe on every call

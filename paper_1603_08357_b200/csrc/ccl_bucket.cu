@@ -369,11 +369,18 @@ static const BucketGrids& bucket_grids()
     return g;
 }
 
-int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, cudaStream_t st, BucketPlan* plan, void** ws_out)
+// region size: 2^23 sites (32 MiB of labels) unless that would need more than kMaxRegions regions
+int bucket_region_shift(int64_t n_sites, const Tuning& t)
 {
-    // region size: 2^23 sites (32 MiB of labels) unless that would need more than kMaxRegions regions
     int shift = t.region_shift;
     while (((n_sites - 1) >> shift) + 1 > kMaxRegions) ++shift;
+    return shift;
+}
+
+int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, int pool_doublings, cudaStream_t st, BucketPlan* plan,
+                   void** ws_out)
+{
+    const int shift = bucket_region_shift(n_sites, t);
     const int n_regions = (int)(((n_sites - 1) >> shift) + 1);
     // Pool: room for 1.25 pairs per bond (every occupied bond, and what the descent re-files) in chunks of about 1/64 of
     // that, plus the chunk every region leaves partly filled.
@@ -381,7 +388,8 @@ int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, cudaStream
     while (cshift < kMaxChunkShift && (n_bonds >> (cshift + 6)) > 0) ++cshift;
     unsigned long long n_chunks;
     if (t.bucket_capacity > 0) n_chunks = (((unsigned long long)t.bucket_capacity - 1) >> cshift) + 1;
-    else n_chunks = (((unsigned long long)n_bonds * 5 / 4) >> cshift) + (unsigned long long)n_regions + 2;
+    else n_chunks = ((((unsigned long long)n_bonds * 5 / 4) << (pool_doublings < 0 ? 0 : pool_doublings > 3 ? 3 : pool_doublings)) >> cshift) +
+                    (unsigned long long)n_regions + 2;
     if (n_chunks > 0x7FFFFFF0ull) n_chunks = 0x7FFFFFF0ull;
     const size_t hdr_bytes = (sizeof(BucketHeader) + 255) & ~(size_t)255;
     const size_t table_bytes = (((size_t)n_regions * n_chunks * sizeof(unsigned int)) + 255) & ~(size_t)255;

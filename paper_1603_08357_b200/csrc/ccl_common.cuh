@@ -143,7 +143,9 @@ struct BucketPlan {
 };
 // bucketed_begin allocates and clears the workspace (*ws_out: the caller frees it with cudaFreeAsync after the last
 // kernel that reads it has been enqueued); bucketed_launch enqueues k_scatter and one k_descend per region.
-int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, cudaStream_t st, BucketPlan* plan, void** ws_out);
+int bucket_region_shift(int64_t n_sites, const Tuning& t);
+int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, int pool_doublings, cudaStream_t st, BucketPlan* plan,
+                   void** ws_out);
 int bucketed_launch(const BucketPlan& plan, int64_t n_sites, int64_t n_bonds, const int32_t* src, const int32_t* dst,
                     const void* occ, int mask_kind, int32_t* labels, cudaStream_t st);
 

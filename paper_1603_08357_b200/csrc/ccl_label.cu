@@ -126,11 +126,18 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
 template <int MASK, bool VEC>
 __global__ void __launch_bounds__(kThreads)
 k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, int gate, int premerge)
+         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, int gate, int premerge,
+         int32_t* notify, int32_t notify_value)
 {
     __shared__ int2 queue[kThreads / 32][128];
     pdl_wait();
     if (!gate_open(hdr, gate)) return;                     // the bucketed form (ccl_bucket.cu) did step (iii)
+    // Running as the safety net of the bucketed form (its chunk pool ran dry): tell the host, through mapped pinned
+    // memory, that the next call on this bond list should draw a larger pool (label_impl).
+    if (notify != nullptr && hdr != nullptr && hdr->overflow != 0 && blockIdx.x == 0 && threadIdx.x == 0) {
+        *reinterpret_cast<volatile int32_t*>(notify) = notify_value;
+        __threadfence_system();
+    }
     const uint64_t pol = evict_first_policy();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
@@ -356,7 +363,8 @@ static int check_args(int64_t n_sites, int64_t n_bonds, const void* src, const v
 
 template <int MASK>
 static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst, const void* occ,
-                         int32_t* labels, const BucketHeader* hdr, int gate, cudaStream_t st)
+                         int32_t* labels, const BucketHeader* hdr, int gate, cudaStream_t st, int32_t* notify = nullptr,
+                         int32_t notify_value = 0)
 {
     const int64_t groups = (n_bonds + 3) / 4;
     int64_t blocks = (groups + kThreads - 1) / kThreads;
@@ -365,8 +373,8 @@ static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     bool vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
-    if (vec) CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, true>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, pm));
-    else     CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, false>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, pm));
+    if (vec) CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, true>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, pm, notify, notify_value));
+    else     CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, false>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, pm, notify, notify_value));
     count_launch();
     return CCL_OK;
 }
@@ -443,7 +451,9 @@ struct ProbeHint {
     const void* dst = nullptr;
     int64_t n_bonds = 0, n_sites = 0;
     int shift = 0;
-    int32_t* answer = nullptr;                     // pinned; -1 until the copy has landed
+    int32_t* answer = nullptr;                     // pinned, two words: [0] the probe's answer, -1 until the copy has landed;
+                                                   // [1] how often the chunk pool ran dry on this bond list (written by the
+                                                   // device: the pool of the next call is doubled that many times)
 };
 static thread_local ProbeHint g_hints[4];
 static thread_local int g_hint_next = 0;
@@ -459,12 +469,13 @@ static ProbeHint* hint_new(const void* src, const void* dst, int64_t n_bonds, in
 {
     ProbeHint& h = g_hints[g_hint_next];
     g_hint_next = (g_hint_next + 1) % 4;
-    if (h.answer == nullptr && cudaHostAlloc(reinterpret_cast<void**>(&h.answer), sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) {
+    if (h.answer == nullptr && cudaHostAlloc(reinterpret_cast<void**>(&h.answer), 2 * sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) {
         h.answer = nullptr;
         cudaGetLastError();
         return nullptr;
     }
-    *reinterpret_cast<volatile int32_t*>(h.answer) = -1;
+    reinterpret_cast<volatile int32_t*>(h.answer)[0] = -1;
+    reinterpret_cast<volatile int32_t*>(h.answer)[1] = 0;
     h.src = src; h.dst = dst; h.n_bonds = n_bonds; h.n_sites = n_sites; h.shift = shift;
     return &h;
 }
@@ -487,20 +498,23 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
     bool report_probe = false;
     const bool eligible = n_bonds > 0 && t.force_mode != 0 && n_sites * (int64_t)sizeof(int32_t) >= t.bucket_min_label_bytes &&
                           n_bonds >= t.bucket_min_bonds;
+    int pool_doublings = 0;
     if (eligible) {
-        rc = bucketed_begin(n_sites, n_bonds, t, st, &plan, &bucket_ws);
-        if (rc != CCL_OK) return rc;
         mode = t.force_mode == 1 ? 1 : -1;
-        if (mode < 0 && t.probe_cache) {
-            hint = hint_find(src, dst, n_bonds, n_sites, plan.shift);
+        if (t.probe_cache) {
+            const int shift = bucket_region_shift(n_sites, t);
+            hint = hint_find(src, dst, n_bonds, n_sites, shift);
             if (hint) {
-                const int32_t ans = *reinterpret_cast<volatile int32_t*>(hint->answer);
-                if (ans == 0 || ans == 1) mode = ans;
+                const int32_t ans = reinterpret_cast<volatile int32_t*>(hint->answer)[0];
+                if (mode < 0 && (ans == 0 || ans == 1)) mode = ans;
+                pool_doublings = reinterpret_cast<volatile int32_t*>(hint->answer)[1];
             } else {
-                hint = hint_new(src, dst, n_bonds, n_sites, plan.shift);
-                report_probe = hint != nullptr;
+                hint = hint_new(src, dst, n_bonds, n_sites, shift);
+                report_probe = hint != nullptr && mode < 0;
             }
         }
+        rc = bucketed_begin(n_sites, n_bonds, t, pool_doublings, st, &plan, &bucket_ws);
+        if (rc != CCL_OK) return rc;
     }
     auto done = [&](int code) { if (bucket_ws) cudaFreeAsync(bucket_ws, st); return code; };
     const int gate = mode < 0 ? kGateDirectOrOverflow : kGateOverflow;
@@ -534,9 +548,13 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
             if (occ == nullptr) rc = launch_two_pass<0>(n_sites, n_bonds, src, dst, nullptr, labels, hdr, g, st);
             else if (mask_kind == 1) rc = launch_two_pass<1>(n_sites, n_bonds, src, dst, occ, labels, hdr, g, st);
             else rc = launch_two_pass<2>(n_sites, n_bonds, src, dst, occ, labels, hdr, g, st);
-        } else if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, hdr, g, st);
-        else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, hdr, g, st);
-        else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, hdr, g, st);
+        } else {
+            // (the safety net reports a dry pool to the host: the next call on this bond list doubles it, up to 8 x)
+            int32_t* notify = (hint != nullptr && mode != 0 && t.bucket_capacity <= 0 && pool_doublings < 3) ? hint->answer + 1 : nullptr;
+            if (occ == nullptr) rc = launch_reduce<0>(n_bonds, src, dst, nullptr, labels, hdr, g, st, notify, pool_doublings + 1);
+            else if (mask_kind == 1) rc = launch_reduce<1>(n_bonds, src, dst, occ, labels, hdr, g, st, notify, pool_doublings + 1);
+            else rc = launch_reduce<2>(n_bonds, src, dst, occ, labels, hdr, g, st, notify, pool_doublings + 1);
+        }
         if (rc != CCL_OK) return done(rc);
         mark(1, st);
         // ---- step (iv)

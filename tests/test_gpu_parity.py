@@ -403,6 +403,31 @@ def test_scratch_is_reported_and_can_be_trimmed(ccl):
     ccl.trim_scratch(0)
 
 
+def test_chunk_pool_grows_after_running_dry(ccl):
+    """The pair pool of the bucketed form holds 1.25 pairs per bond.  A densely occupied random graph files about 2.5: the
+    first call runs dry and is finished by the direct kernel behind the bucketed kernels, which also tells the host; the
+    next calls on the same bond list draw a pool twice (four, eight times) as large.  Labels are right every time."""
+    torch.cuda.synchronize()
+    ccl.trim_scratch(0)
+    ccl.set_tuning(0, 16, 1, 0)                            # bucketed form, 2^16-site regions, default pool size
+    rng = np.random.default_rng(808)
+    n, m = 1 << 20, 1 << 22                                # (large enough for the pool's 32 MiB granules to show)
+    src, dst = graphs.random_graph(rng, n, m)
+    s, d = dev(src), dev(dst)
+    want = oracle.label(n, src, dst)
+    reserved = []
+    for rep in range(5):
+        got = ccl.label(n, s, d)                           # every bond occupied
+        torch.cuda.synchronize()
+        assert np.array_equal(got.cpu().numpy(), want), rep
+        reserved.append(ccl.scratch_bytes()[0])
+    assert reserved[1] > reserved[0]                       # the second call drew a larger pool
+    assert reserved[-1] == reserved[-2]                    # ... and it stops growing once nothing is dropped
+    assert reserved[-1] <= 8 * reserved[0]
+    ccl.set_tuning()
+    ccl.trim_scratch(0)
+
+
 def test_probe_cache_on_and_off(ccl):
     """The host-side memory of the device probe's answer changes which kernels are enqueued, never the labels: repeated
     calls on one bond list (first call: probe undecided, later calls: decided) and the same with the cache off."""
