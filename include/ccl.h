@@ -208,14 +208,15 @@ int ccl_scratch_bytes(int64_t* reserved, int64_t* in_use);
  *                             re-does the bond list behind the bucketed kernels
  *   "scatter_tiles"           1 = the bulk-copy (cp.async.bulk) scatter kernel for 16-byte aligned input (default),
  *                             0 = the register kernel for everything
- *   "probe_cache"             1 = remember the probe's answer per bond list (default), 0 = probe on every call
+ *   "probe_cache"             1 = remember the probe's answer per bond list (default), 0 = probe on every call;
+ *                             setting it (either way) forgets what this thread remembers about earlier bond lists
  *   "two_pass"                direct form of step (iii): 0 = one pass over the bonds, 1 = the paper's order of work
  *                             (hook every site to its smallest lower neighbour, flatten, then Algorithm 1; two passes
  *                             over the bonds), -1 = two passes iff n_bonds >= 2.5 n_sites and n_bonds >= 2^20 (default)
  *   "flatten_window_bytes"    step (iv) behind the bucketed form gathers from one window of label[] of this many bytes
  *                             at a time (default 64 MiB, what stays resident in L2);
  *   "flatten_window_min_bytes" ... for label arrays of at least this many bytes (default 96 MiB; 0 = always; < 0 = never)
- *   "reset"                   all defaults (value ignored)
+ *   "reset"                   all defaults (value ignored); also forgets the remembered bond lists
  * Unknown names -> CCL_INVALID_ARG. */
 int ccl_set_option(const char* name, int64_t value);
 

@@ -72,7 +72,7 @@ extern "C" int ccl_set_option(const char* name, int64_t value)
     ccl::Tuning def;
     ccl::Tuning& t = ccl::tuning();
     if (name == nullptr) { ccl::set_error("invalid argument: option name is NULL"); return CCL_INVALID_ARG; }
-    if (!strcmp(name, "reset")) { t = def; return CCL_OK; }
+    if (!strcmp(name, "reset")) { t = def; ccl::forget_probe_hints(); return CCL_OK; }
     if (!strcmp(name, "bucket_min_label_bytes")) {
         t.bucket_min_label_bytes = value >= 0 ? value : def.bucket_min_label_bytes;
         t.bucket_min_bonds = value >= 0 ? 0 : def.bucket_min_bonds;
@@ -98,7 +98,7 @@ extern "C" int ccl_set_option(const char* name, int64_t value)
     if (!strcmp(name, "two_pass")) { t.two_pass = value > 0 ? 1 : value < 0 ? -1 : 0; return CCL_OK; }
     if (!strcmp(name, "warp_premerge")) { t.warp_premerge = value != 0; return CCL_OK; }
     if (!strcmp(name, "scatter_tiles")) { t.scatter_tiles = value != 0; return CCL_OK; }
-    if (!strcmp(name, "probe_cache")) { t.probe_cache = value != 0; return CCL_OK; }
+    if (!strcmp(name, "probe_cache")) { t.probe_cache = value != 0; ccl::forget_probe_hints(); return CCL_OK; }
     if (!strcmp(name, "flatten_window_bytes")) {
         t.flatten_window_bytes = value > 0 ? value : def.flatten_window_bytes;
         return CCL_OK;

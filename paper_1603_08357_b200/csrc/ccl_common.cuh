@@ -118,6 +118,8 @@ struct Tuning {                                    // ccl_set_option(); one set 
 };
 Tuning& tuning();
 
+void forget_probe_hints();                         // ccl_label.cu: drops this host thread's per-bond-list memory (R15)
+
 // The library's own stream-ordered memory pool on the current device (created on first use; ccl_trim_scratch returns
 // what it holds to the driver), so scratch freed by one call is reused by the next.
 int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st);

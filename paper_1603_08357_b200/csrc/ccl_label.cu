@@ -465,6 +465,13 @@ static ProbeHint* hint_find(const void* src, const void* dst, int64_t n_bonds, i
     return nullptr;
 }
 
+// ccl_set_option("probe_cache" | "reset"): what this host thread remembers about bond lists is forgotten (the pinned
+// words are kept for reuse)
+void forget_probe_hints()
+{
+    for (ProbeHint& h : g_hints) { h.src = nullptr; h.dst = nullptr; h.n_bonds = -1; }
+}
+
 static ProbeHint* hint_new(const void* src, const void* dst, int64_t n_bonds, int64_t n_sites, int shift)
 {
     ProbeHint& h = g_hints[g_hint_next];
