@@ -453,6 +453,12 @@ def test_probe_cache_on_and_off(ccl):
                 assert np.array_equal(got.cpu().numpy(), oracle.label(n, src, dst, mask)), (local, cache, rep)
             if cache and local:
                 assert counts[-1] < counts[0]              # once decided, only the chosen (direct) form is enqueued
+                ccl.set_option("probe_cache", 1)           # setting the option forgets the remembered bond lists
+                before = ccl.launch_count()
+                got = ccl.label(n, s, d, dev(mask))
+                torch.cuda.synchronize()
+                assert ccl.launch_count() - before == counts[0]        # ... so this is a first call again
+                assert np.array_equal(got.cpu().numpy(), oracle.label(n, src, dst, mask))
             elif not cache:
                 assert counts[-1] == counts[0]
     ccl.set_option("reset")
