@@ -130,6 +130,28 @@ int ccl_gen_occupancy(int64_t n_bonds, double p, uint64_t seed, uint32_t realiza
 int ccl_cluster_stats(int64_t n_sites, const int32_t* labels, int32_t* size_scratch, ccl_stats* out,
                       int64_t* hist_dense, int32_t n_dense, int64_t* hist_log2, void* stream);
 
+/* ---- the same statistics without any device allocation ------------------------------------------------
+ *
+ * For callers that cannot allocate device memory and so cannot bring the size_scratch ccl_cluster_stats asks for:
+ * a program that gave the whole GPU to its own memory arena at start-up (cudaMalloc would fail), or a loop that must
+ * not issue cudaMalloc / cudaFree because both synchronise the device and stall every other stream of the process.
+ * The per-label size table lives in a fixed array inside the library image instead: CCL_STATS_STATIC_MAX_SITES int32
+ * counters = 16 MiB, held on every GPU that loads libccl.so from module load until the process exits.  The call
+ * itself issues no cudaMalloc, cudaFree, memory-pool or other allocating call; it enqueues memsets and the kernels
+ * of ccl_cluster_stats on `stream`.  labels, out, hist_dense, n_dense, hist_log2: as for ccl_cluster_stats, all
+ * caller-owned device memory; same results.
+ *   - n_sites > CCL_STATS_STATIC_MAX_SITES -> CCL_INVALID_ARG (checked on the host before anything is enqueued;
+ *     use ccl_cluster_stats with your own scratch for larger label arrays).
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *     current) and caches it; make that first call during set-up, before any stream capture is begun.
+ *   - Every call on a device uses the SAME array.  The call clears the n_sites counters it needs, so earlier
+ *     contents never leak into a result, but two calls whose kernels overlap on the GPU (different streams, or
+ *     different host threads on different streams) race on it and both results are garbage: keep calls on one
+ *     device in one stream order. */
+#define CCL_STATS_STATIC_MAX_SITES (1 << 22)
+int ccl_cluster_stats_static(int64_t n_sites, const int32_t* labels, ccl_stats* out, int64_t* hist_dense,
+                             int32_t n_dense, int64_t* hist_log2, void* stream);
+
 /* ---- whole-call convenience with HOST buffers (the end-to-end path bench.py times as "e2e") ----------
  *
  * Copies src/dst/occupied_bits from host memory (pinned for full speed) to device scratch the call allocates and

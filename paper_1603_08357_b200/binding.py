@@ -16,7 +16,7 @@ EXPORTS = ["ccl_label", "ccl_label_bits", "ccl_validate_bonds", "ccl_gen_triangu
            "ccl_gen_regular", "ccl_gen_occupancy", "ccl_cluster_stats", "ccl_label_bits_host",
            "ccl_set_profile_events", "ccl_set_option", "ccl_label_batch", "ccl_relabel_sequential", "ccl_gen_cayley3",
            "ccl_gen_wrap_vectors", "ccl_wrap", "ccl_label_nn", "ccl_label_sweep_host", "ccl_trim_scratch",
-           "ccl_scratch_bytes", "ccl_last_error", "ccl_version", "ccl_launch_count"]
+           "ccl_scratch_bytes", "ccl_cluster_stats_static", "ccl_last_error", "ccl_version", "ccl_launch_count"]
 
 _vp, _i64, _i32, _u64, _u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
 lib.ccl_label.argtypes = [_i64, _i64, _vp, _vp, _vp, _vp, _vp]
@@ -28,6 +28,7 @@ lib.ccl_gen_honeycomb.argtypes = [_i32, _vp, _vp, _vp]
 lib.ccl_gen_regular.argtypes = [_i64, _i32, _u64, _vp, _vp, _vp, C.POINTER(C.c_size_t), _vp]
 lib.ccl_gen_occupancy.argtypes = [_i64, C.c_double, _u64, _u32, _vp, _vp, _vp]
 lib.ccl_cluster_stats.argtypes = [_i64, _vp, _vp, _vp, _vp, _i32, _vp, _vp]
+lib.ccl_cluster_stats_static.argtypes = [_i64, _vp, _vp, _vp, _i32, _vp, _vp]
 lib.ccl_last_error.restype = C.c_char_p
 lib.ccl_last_error.argtypes = []
 lib.ccl_version.argtypes = []
@@ -44,7 +45,7 @@ lib.ccl_label_nn.argtypes = [_i64, _i32, _vp, _vp, _vp]
 lib.ccl_label_sweep_host.argtypes = [_i64, _i64, _vp, _vp, _i32, _vp, _vp, _vp]
 lib.ccl_trim_scratch.argtypes = [C.c_size_t, _vp]
 lib.ccl_scratch_bytes.argtypes = [C.POINTER(_i64), C.POINTER(_i64)]
-for _n in EXPORTS[:20]:
+for _n in EXPORTS[:21]:
     getattr(lib, _n).restype = C.c_int
 
 
@@ -314,6 +315,31 @@ def cluster_stats(labels, n_dense=0):
     hl = torch.empty(32, dtype=torch.int64, device=dev)
     _check(lib.ccl_cluster_stats(n, _dev(labels, torch.int32, "labels"), scratch.data_ptr(), out.data_ptr(),
                                  hd.data_ptr(), n_dense, hl.data_ptr(), _stream()), "ccl_cluster_stats")
+    o = out.cpu().tolist()
+    d = dict(n_clusters=o[0], largest=o[1], largest_label=o[2], sum_s2=o[3] & 0xFFFFFFFFFFFFFFFF)
+    return d, hd.cpu(), hl.cpu()
+
+
+STATS_STATIC_MAX_SITES = 1 << 22       # CCL_STATS_STATIC_MAX_SITES of include/ccl.h
+
+
+def cluster_stats_static(labels, n_dense=0, out=None, hist_dense=None, hist_log2=None):
+    """ccl_cluster_stats_static: cluster_stats for callers that cannot allocate device memory (all of it belongs to
+    their own arena, or a cudaMalloc's device-wide synchronisation is not acceptable where they call from).  The size
+    table sits in a fixed 16 MiB array inside libccl.so, so at most STATS_STATIC_MAX_SITES labels; the library call
+    allocates nothing.  Pass `out` (int64[4]), `hist_dense` (int64[n_dense+1]) and `hist_log2` (int64[32]) CUDA
+    tensors to keep this wrapper from allocating the outputs as well.  Calls on one device share the array: do not
+    let two of them overlap on the GPU.  Returns like cluster_stats (synchronises to read back)."""
+    n = labels.numel()
+    dev = labels.device
+    out = torch.empty(4, dtype=torch.int64, device=dev) if out is None else out
+    hd = torch.empty(n_dense + 1, dtype=torch.int64, device=dev) if hist_dense is None else hist_dense
+    hl = torch.empty(32, dtype=torch.int64, device=dev) if hist_log2 is None else hist_log2
+    if out.numel() < 4 or hd.numel() < n_dense + 1 or hl.numel() < 32:
+        raise ValueError("ccl_cluster_stats_static: an output tensor is too short")
+    _check(lib.ccl_cluster_stats_static(n, _dev(labels, torch.int32, "labels"), _dev(out, torch.int64, "out"),
+                                        _dev(hd, torch.int64, "hist_dense"), n_dense,
+                                        _dev(hl, torch.int64, "hist_log2"), _stream()), "ccl_cluster_stats_static")
     o = out.cpu().tolist()
     d = dict(n_clusters=o[0], largest=o[1], largest_label=o[2], sum_s2=o[3] & 0xFFFFFFFFFFFFFFFF)
     return d, hd.cpu(), hl.cpu()

@@ -52,6 +52,10 @@ def test_argument_checking_is_host_side():
     need = C.c_size_t(0)
     assert lib.ccl_gen_regular(5, 3, 1, None, None, None, C.byref(need), None) == 1     # odd stub count
     assert lib.ccl_cluster_stats(-1, None, None, p, None, 0, None, None) == 1
+    # the no-allocation variant refuses label arrays beyond its fixed table before it touches the device
+    assert lib.ccl_cluster_stats_static(binding.STATS_STATIC_MAX_SITES + 1, p, p, None, 0, None, None) == 1
+    assert "CCL_STATS_STATIC_MAX_SITES" in binding.last_error()
+    assert lib.ccl_cluster_stats_static(-1, p, p, None, 0, None, None) == 1
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
