@@ -17,7 +17,9 @@
  *     pay the driver for memory each time) until ccl_trim_scratch() hands it back; ccl_scratch_bytes() reports it.
  *     What a call draws: ccl_label / ccl_label_bits nothing, unless n_sites * 4 >= 96 MiB and n_bonds >= 2^20 (the
  *     region-bucketed form): then 10 * n_bonds bytes of pair chunks plus a table (about 1.5 GB for 2^27 bonds; twice,
- *     four, at most eight times that on a bond list on which an earlier call ran the pool dry);
+ *     four, at most eight times that on a bond list on which an earlier call ran the pool dry) -- except that a call
+ *     on a bond list for which the remembered probe answer is "direct" draws nothing, and that a call whose workspace
+ *     cannot be allocated does not fail: it runs the direct kernels, which need none;
  *     the host-buffer entry points also their device copies of src, dst, masks and labels.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the default stream).  All work is enqueued on it; no
  *     entry point synchronises with the host unless stated.  Results are valid once the stream has drained.
@@ -78,7 +80,8 @@ int ccl_label_bits(int64_t n_sites, int64_t n_bonds, const int32_t* src, const i
  * entries are padding.  Every entry is a connection of the network to be labeled; a bond may be listed at both of its
  * ends (the paper's form) or at either one.
  * The four steps run in the paper's form: (i) label[i] = smallest lower-numbered neighbour, else i; (ii) analysis;
- * (iii) Algorithm 1 over every (site, lower-numbered neighbour); (iv) analysis.  Same result as ccl_label on the
+ * (iii) Algorithm 1 over every listed entry (site i, neighbour j != i), whichever of the two is lower -- so a bond listed
+ * at one end only is still joined; (iv) analysis.  Same result as ccl_label on the
  * corresponding bond list.  0 <= z_max <= 1024; neighbours >= n_sites are a caller error (not checked). */
 int ccl_label_nn(int64_t n_sites, int32_t z_max, const int32_t* nn_list, int32_t* labels, void* stream);
 

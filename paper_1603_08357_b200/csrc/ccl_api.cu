@@ -2,6 +2,7 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <atomic>
 #include <mutex>
 
 #include "ccl_common.cuh"
@@ -25,6 +26,19 @@ Tuning& tuning()
 {
     static thread_local Tuning t;                  // per host thread, like the error string and the launch counter
     return t;
+}
+
+int sm_count()
+{
+    static std::atomic<int> cached[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return 148; }
+    int n = cached[dev].load(std::memory_order_relaxed);
+    if (n <= 0) {
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) { cudaGetLastError(); return 148; }
+        cached[dev].store(n, std::memory_order_relaxed);
+    }
+    return n;
 }
 
 static std::mutex g_pool_mutex;
@@ -96,7 +110,6 @@ extern "C" int ccl_set_option(const char* name, int64_t value)
     }
     if (!strcmp(name, "bucket_capacity")) { t.bucket_capacity = value > 0 ? value : 0; return CCL_OK; }
     if (!strcmp(name, "two_pass")) { t.two_pass = value > 0 ? 1 : value < 0 ? -1 : 0; return CCL_OK; }
-    if (!strcmp(name, "warp_premerge")) { t.warp_premerge = value != 0; return CCL_OK; }
     if (!strcmp(name, "scatter_tiles")) { t.scatter_tiles = value != 0; return CCL_OK; }
     if (!strcmp(name, "probe_cache")) { t.probe_cache = value != 0; ccl::forget_probe_hints(); return CCL_OK; }
     if (!strcmp(name, "flatten_window_bytes")) {

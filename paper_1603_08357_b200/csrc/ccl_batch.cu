@@ -159,7 +159,7 @@ extern "C" int ccl_relabel_sequential(int64_t n_sites, const int32_t* labels, in
     int32_t* rank = reinterpret_cast<int32_t*>(static_cast<char*>(workspace) + arr);
     void* tmp = static_cast<char*>(workspace) + 2 * arr;
     int64_t blocks = (n_sites + 255) / 256;
-    if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+    if (blocks > (int64_t)sm_count() * 16) blocks = (int64_t)sm_count() * 16;
     k_flag_roots<<<(unsigned)blocks, 256, 0, st>>>(n_sites, labels, flag);
     CCL_CHECK_LAUNCH("k_flag_roots");
     CCL_CUDA_TRY(cub::DeviceScan::ExclusiveSum(tmp, temp, flag, rank, (int)n_sites, st));

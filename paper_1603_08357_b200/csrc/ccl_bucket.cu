@@ -20,6 +20,8 @@
 // Step (i) rides along: label[] of region r is written (label[i] = i) by the kernel that runs just before
 // k_descend(r), so the lines are still in L2 when the first atomic arrives, and the write to HBM and the fetch back
 // that a separate initialization pass costs disappear.
+#include <mutex>
+
 #include "ccl_common.cuh"
 #include "ccl_unionfind.cuh"
 #include "ccl_emit.cuh"
@@ -238,7 +240,7 @@ k_scatter_tiles(int64_t n_tiles, const int32_t* __restrict__ src, const int32_t*
 // Reduce region r: all label[] traffic of this launch falls into [r << shift, (r+1) << shift).  init_lo < init_hi: the
 // labels of the region that comes next are written on the way out (step (i) for that region).
 __global__ void __launch_bounds__(kBThreads, 8)
-k_descend(int r, BucketRef bk, int gated, int64_t init_lo, int64_t init_hi, int premerge, int32_t* label)
+k_descend(int r, BucketRef bk, int gated, int64_t init_lo, int64_t init_hi, int32_t* label)
 {
     constexpr int P = kDescendP;
     __shared__ EmitSmem sm;
@@ -299,32 +301,12 @@ k_descend(int r, BucketRef bk, int gated, int64_t init_lo, int64_t init_hi, int 
                     else v[k] = label[nb];
                 }
             }
-            if (premerge) {
-                // Experiment (ccl_set_option "warp_premerge", off by default; profiles/r2_premerge.md): lanes whose
-                // atomics target the same site b elect the smallest partner; one lane links b to it, the others go on
-                // with {a_min, a} as if they had read label[b] = a_min.
-                const int lane = threadIdx.x & 31;
 #pragma unroll
-                for (int k = 0; k < P; ++k) {
-                    const bool need = act[k] && v[k] > a[k];
-                    const unsigned peers = __match_any_sync(0xffffffffu, need ? b[k] : ~lane);
-                    const int32_t amin = __reduce_min_sync(peers, a[k]);
-                    const unsigned mins = __ballot_sync(0xffffffffu, a[k] == amin) & peers;
-                    if (act[k]) {
-                        if (!need) old[k] = v[k];
-                        else if (lane == __ffs(mins) - 1) old[k] = atomicMin(label + b[k], a[k]);
-                        else old[k] = amin;
-                    }
-                }
-            } else {
-#pragma unroll
-                for (int k = 0; k < P; ++k)
-                    if (act[k]) old[k] = (v[k] > a[k]) ? atomicMin(label + b[k], a[k]) : v[k];
-            }
+            for (int k = 0; k < P; ++k)
+                if (act[k]) old[k] = (v[k] > a[k]) ? atomicMin(label + b[k], a[k]) : v[k];
 #pragma unroll
             for (int k = 0; k < P; ++k)
                 if (act[k]) { act[k] = old[k] != b[k] && old[k] != a[k]; any |= act[k]; }
-            if (premerge) any = __any_sync(0xffffffffu, any);          // the pre-merge needs the whole warp in step
             if (!any) break;
         }
         bool pending = false;
@@ -347,26 +329,43 @@ static int resident_grid(K kernel, size_t smem)
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kBThreads, smem) != cudaSuccess) per_sm = 0;
     cudaGetLastError();
     if (per_sm < 1) per_sm = 1;
-    int sms = kSMs, dev = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    return per_sm * (sms > 0 ? sms : kSMs);
+    return per_sm * sm_count();
 }
 
-struct BucketGrids { int scatter = 0, tiles[3] = {0, 0, 0}, descend = 0; };
-static const BucketGrids& bucket_grids()
+// The grids -- and the opt-in to more than 48 KB of dynamic shared memory that k_scatter_tiles needs -- belong to a
+// device, not to the process: one entry per device, filled under a lock by the first eligible call on that device.
+struct BucketGrids { bool ready = false; int scatter = 0, tiles[3] = {0, 0, 0}, descend = 0; };
+static std::mutex g_grids_mutex;
+static BucketGrids g_grids[64];
+
+template <int MASK>
+static int tiles_grid()
 {
-    static BucketGrids g;
-    if (g.descend == 0) {
-        g.scatter = resident_grid(k_scatter<2>, 0);
-        cudaFuncSetAttribute(k_scatter_tiles<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem<0>));
-        cudaFuncSetAttribute(k_scatter_tiles<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem<1>));
-        cudaFuncSetAttribute(k_scatter_tiles<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem<2>));
-        g.tiles[0] = resident_grid(k_scatter_tiles<0>, sizeof(ScatterSmem<0>));
-        g.tiles[1] = resident_grid(k_scatter_tiles<1>, sizeof(ScatterSmem<1>));
-        g.tiles[2] = resident_grid(k_scatter_tiles<2>, sizeof(ScatterSmem<2>));
-        g.descend = resident_grid(k_descend, 0);
+    // 0 = the opt-in failed on this device: the register kernel (k_scatter) takes the whole bond list instead
+    if (cudaFuncSetAttribute(k_scatter_tiles<MASK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem<MASK>)) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
     }
-    return g;
+    return resident_grid(k_scatter_tiles<MASK>, sizeof(ScatterSmem<MASK>));
+}
+
+static int bucket_grids(BucketGrids* out)
+{
+    int dev = 0;
+    CCL_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) { set_error("device index %d out of range", dev); return CCL_UNSUPPORTED; }
+    std::lock_guard<std::mutex> lock(g_grids_mutex);
+    BucketGrids& g = g_grids[dev];
+    if (!g.ready) {
+        g.scatter = resident_grid(k_scatter<2>, 0);
+        g.tiles[0] = tiles_grid<0>();
+        g.tiles[1] = tiles_grid<1>();
+        g.tiles[2] = tiles_grid<2>();
+        g.descend = resident_grid(k_descend, 0);
+        g.ready = true;
+    }
+    *out = g;
+    return CCL_OK;
 }
 
 // region size: 2^23 sites (32 MiB of labels) unless that would need more than kMaxRegions regions
@@ -406,7 +405,6 @@ int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, int pool_d
     plan->cshift = cshift;
     plan->n_regions = n_regions;
     plan->scatter_tiles = t.scatter_tiles;
-    plan->premerge = t.warp_premerge;
     CCL_CUDA_TRY(cudaMemsetAsync(ws, 0, hdr_bytes + table_bytes, st));
     return CCL_OK;
 }
@@ -420,14 +418,15 @@ int bucketed_launch(const BucketPlan& plan, int64_t n_sites, int64_t n_bonds, co
     const int R = plan.n_regions, shift = plan.shift;
     const uintptr_t al = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     const int vec = (al & 15) == 0;
-    const BucketGrids& grids = bucket_grids();
+    BucketGrids grids;
+    { const int rc = bucket_grids(&grids); if (rc != CCL_OK) return rc; }
     const int mk = occ == nullptr ? 0 : mask_kind;
     // the top region must hold label[i] = i before the first k_descend touches it; every k_descend writes the labels
     // of the region that comes next
     if (plan.lazy_init) {
         const int64_t lo = (int64_t)(R - 1) << shift;
         int64_t blocks = ((n_sites - lo + 3) / 4 + kBThreads - 1) / kBThreads;
-        if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+        if (blocks > (int64_t)sm_count() * 16) blocks = (int64_t)sm_count() * 16;
         k_init_top<<<(unsigned)blocks, kBThreads, 0, st>>>(lo, n_sites, labels);
         CCL_CHECK_LAUNCH("k_init_top");
     }
@@ -436,7 +435,7 @@ int bucketed_launch(const BucketPlan& plan, int64_t n_sites, int64_t n_bonds, co
     // the register kernel
     int64_t done = 0;
     const bool mask_ok = occ == nullptr || (reinterpret_cast<uintptr_t>(occ) & 15) == 0;
-    if (vec && mask_ok && plan.scatter_tiles && n_bonds >= kTileBonds) {
+    if (vec && mask_ok && plan.scatter_tiles && n_bonds >= kTileBonds && grids.tiles[mk] > 0) {
         const int64_t n_tiles = n_bonds / kTileBonds;
         int tg = grids.tiles[mk];
         if (tg > n_tiles) tg = (int)n_tiles;
@@ -464,7 +463,7 @@ int bucketed_launch(const BucketPlan& plan, int64_t n_sites, int64_t n_bonds, co
             init_hi = (int64_t)r << shift;
             if (init_hi > n_sites) init_hi = n_sites;
         }
-        CCL_CUDA_TRY(launch_pdl(k_descend, (unsigned)grids.descend, (unsigned)kBThreads, st, r, bk, gated, init_lo, init_hi, plan.premerge, labels));
+        CCL_CUDA_TRY(launch_pdl(k_descend, (unsigned)grids.descend, (unsigned)kBThreads, st, r, bk, gated, init_lo, init_hi, labels));
         count_launch();
     }
     return CCL_OK;

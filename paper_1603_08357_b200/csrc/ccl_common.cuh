@@ -11,7 +11,9 @@
 
 namespace ccl {
 
-constexpr int kSMs = 148;                 // B200: 2 dies x 74 SMs
+// Number of SMs of the current device (queried once per device and cached; grids are capped at a multiple of it).
+// 148 on B200 (2 dies x 74 SMs), which is also what is assumed should the query fail.
+int sm_count();
 
 // ---- host plumbing ---------------------------------------------------------------------------------------
 void set_error(const char* fmt, ...);
@@ -109,8 +111,6 @@ struct Tuning {                                    // ccl_set_option(); one set 
     int64_t bucket_capacity = 0;                   // pairs the chunk pool can hold; 0 = 5 M / 4 + slack
     int32_t two_pass = -1;                         // direct form of step (iii): 0 one pass (k_reduce), 1 hook + flatten +
                                                    // join (the paper's order), -1 by bonds per site (>= 2.5: two passes)
-    int32_t warp_premerge = 0;                     // experiment: lanes of a warp that target the same site send one atomic
-                                                   // (measured: nothing to merge on random graphs, slower on lattices)
     int32_t scatter_tiles = 1;                     // 1: k_scatter_tiles (bulk copies into shared memory) for aligned input
     int32_t probe_cache = 1;                       // remember the probe's answer per bond list (host side, hint only)
     int64_t flatten_window_bytes = 64ll << 20;     // step (iv) gathers from one L2-resident window of label[] at a time
@@ -139,7 +139,6 @@ struct BucketPlan {
     int shift = 0, n_regions = 0;
     int cshift = kMinChunkShift;                   // chunk = 2^cshift pairs
     int scatter_tiles = 1;
-    int premerge = 0;
     int lazy_init = 0;                             // 1: label[] of region r is written by the kernel that runs before k_descend(r)
     int gated = 0;                                 // 1: the kernels return at once unless hdr->mode == 1 (probe undecided on the host)
 };

@@ -196,7 +196,7 @@ __global__ void k_repair(int64_t n_bonds, uint2 key, int32_t* src, int32_t* dst,
 static inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 static inline int64_t grid_for(int64_t n) {
     int64_t b = (n + kGenThreads - 1) / kGenThreads;
-    const int64_t cap = (int64_t)kSMs * 16;
+    const int64_t cap = (int64_t)sm_count() * 16;
     return b < 1 ? 1 : (b > cap ? cap : b);
 }
 

@@ -42,13 +42,12 @@ __device__ __forceinline__ bool gate_open(const BucketHeader* hdr, int kind)
 template <int MASK, bool VEC>
 __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_t* __restrict__ src,
                                        const int32_t* __restrict__ dst, const void* __restrict__ occ,
-                                       int32_t* label, uint64_t pol, int premerge, int32_t (&pa)[4], int32_t (&pb)[4])
+                                       int32_t* label, uint64_t pol, int32_t (&pa)[4], int32_t (&pb)[4])
 {
     // Loads this thread's (up to) 4 bonds, does the first-touch atomics, and returns how many pairs are left to join;
-    // they are stored in pa[]/pb[] front-packed.  (With the pre-merge experiment on, every lane of the warp stays to the
-    // end: the vote needs them all.)
-    if (b0 >= n_bonds && !premerge) return 0;
-    const int cnt = (b0 >= n_bonds) ? 0 : (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
+    // they are stored in pa[]/pb[] front-packed.
+    if (b0 >= n_bonds) return 0;
+    const int cnt = (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
 
     // occupancy of this thread's 4 bonds -> low 4 bits of m
     uint32_t m = 0xFu;
@@ -66,11 +65,10 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
         }
     }
     m &= (1u << cnt) - 1u;
-    if (m == 0 && !premerge) return 0;
+    if (m == 0) return 0;
 
     int32_t u[4] = {0, 0, 0, 0}, v[4] = {0, 0, 0, 0};
-    if (m == 0) {
-    } else if (VEC && cnt == 4) {
+    if (VEC && cnt == 4) {
         const int4 s = ld_stream_v4(src + b0, pol), d = ld_stream_v4(dst + b0, pol);
         u[0] = s.x; u[1] = s.y; u[2] = s.z; u[3] = s.w;
         v[0] = d.x; v[1] = d.y; v[2] = d.z; v[3] = d.w;
@@ -92,18 +90,7 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
         const int32_t hi = max(u[k], v[k]);
         old[k] = lo[k];                                    // "nothing left to do"
         const bool need = ((m >> k) & 1u) && hi != lo[k];
-        if (premerge) {
-            // experiment ("warp_premerge"): bonds of this warp with the same higher site send one atomic, with the smallest
-            // of their lower sites; the others are left with the pair {that site, their own lower site}
-            const int lane = threadIdx.x & 31;
-            const unsigned peers = __match_any_sync(0xffffffffu, need ? hi : ~lane);
-            const int32_t amin = __reduce_min_sync(peers, lo[k]);
-            const unsigned mins = __ballot_sync(0xffffffffu, lo[k] == amin) & peers;
-            if (need) {
-                if (lane == __ffs(mins) - 1) { const int32_t o = atomicMin(label + hi, lo[k]); old[k] = (o == hi) ? lo[k] : o; }
-                else old[k] = amin;                        // == lo[k] for a duplicate: nothing left to do
-            }
-        } else if (need) {
+        if (need) {
             const int32_t o = atomicMin(label + hi, lo[k]);
             old[k] = (o == hi) ? lo[k] : o;
         }
@@ -126,7 +113,7 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
 template <int MASK, bool VEC>
 __global__ void __launch_bounds__(kThreads)
 k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, int gate, int premerge,
+         const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, int gate,
          int32_t* notify, int32_t notify_value)
 {
     __shared__ int2 queue[kThreads / 32][128];
@@ -144,7 +131,7 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
     const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
     for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
         int32_t pa[4], pb[4];
-        const int n = reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol, premerge, pa, pb);
+        const int n = reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol, pa, pb);
         int incl = n;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -175,7 +162,7 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
 template <int MASK>
 __global__ void __launch_bounds__(kThreads)
 k_hook(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, const void* __restrict__ occ,
-       int vec, int32_t* label, const BucketHeader* hdr, int gate, int premerge)
+       int vec, int32_t* label, const BucketHeader* hdr, int gate)
 {
     pdl_wait();
     if (!gate_open(hdr, gate)) return;                     // another form did step (iii)
@@ -188,14 +175,7 @@ k_hook(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restri
         for (int k = 0; k < 4; ++k) {
             const bool need = ((c.m >> k) & 1u) && c.u[k] != c.v[k];
             const int32_t lo = min(c.u[k], c.v[k]), hi = max(c.u[k], c.v[k]);
-            if (premerge) {                                // experiment ("warp_premerge"): one atomic per distinct higher site
-                const int lane = threadIdx.x & 31;
-                const unsigned peers = __match_any_sync(0xffffffffu, need ? hi : ~lane);
-                const int32_t amin = __reduce_min_sync(peers, lo);
-                if (need && lane == __ffs(peers) - 1) atomicMin(label + hi, amin);
-            } else if (need) {
-                atomicMin(label + hi, lo);
-            }
+            if (need) atomicMin(label + hi, lo);
         }
     }
 }
@@ -368,13 +348,12 @@ static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst
 {
     const int64_t groups = (n_bonds + 3) / 4;
     int64_t blocks = (groups + kThreads - 1) / kThreads;
-    if (blocks > (int64_t)kSMs * 8 * 4) blocks = (int64_t)kSMs * 8 * 4;       // grid-stride beyond 4 waves of 8 CTAs/SM
-    const int pm = tuning().warp_premerge;
+    if (blocks > (int64_t)sm_count() * 8 * 4) blocks = (int64_t)sm_count() * 8 * 4;       // grid-stride beyond 4 waves of 8 CTAs/SM
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     bool vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
-    if (vec) CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, true>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, pm, notify, notify_value));
-    else     CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, false>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, pm, notify, notify_value));
+    if (vec) CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, true>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, notify, notify_value));
+    else     CCL_CUDA_TRY(launch_pdl(k_reduce<MASK, false>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, labels, hdr, gate, notify, notify_value));
     count_launch();
     return CCL_OK;
 }
@@ -395,14 +374,14 @@ static int launch_two_pass(int64_t n_sites, int64_t n_bonds, const int32_t* src,
 {
     const int64_t groups = (n_bonds + 3) / 4;
     int64_t blocks = (groups + kThreads - 1) / kThreads;
-    if (blocks > (int64_t)kSMs * 8 * 4) blocks = (int64_t)kSMs * 8 * 4;
+    if (blocks > (int64_t)sm_count() * 8 * 4) blocks = (int64_t)sm_count() * 8 * 4;
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     int vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
     // hook and the mid-call flatten are this form's own steps (i)/(ii); the join pass also serves as the safety net of
     // the bucketed form (it joins whatever the ends of an occupied bond still differ in)
     const int own = gate == kGateNone ? kGateNone : kGateDirect;
-    CCL_CUDA_TRY(launch_pdl(k_hook<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, own, tuning().warp_premerge));   // step (i), paper form
+    CCL_CUDA_TRY(launch_pdl(k_hook<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, own));   // step (i), paper form
     count_launch();
     { const int rc = launch_flatten(n_sites, labels, 0, n_sites, hdr, own, st); if (rc != CCL_OK) return rc; }                      // step (ii)
     CCL_CUDA_TRY(launch_pdl(k_join<MASK>, (unsigned)blocks, (unsigned)kThreads, st, n_bonds, src, dst, occ, vec, labels, hdr, gate));   // step (iii)
@@ -449,38 +428,52 @@ static inline void mark(int k, cudaStream_t st)
 struct ProbeHint {
     const void* src = nullptr;
     const void* dst = nullptr;
-    int64_t n_bonds = 0, n_sites = 0;
+    int64_t n_bonds = -1, n_sites = 0;
     int shift = 0;
-    int32_t* answer = nullptr;                     // pinned, two words: [0] the probe's answer, -1 until the copy has landed;
-                                                   // [1] how often the chunk pool ran dry on this bond list (written by the
-                                                   // device: the pool of the next call is doubled that many times)
+    int32_t* answer = nullptr;                     // two words of the thread's pinned block: [0] the probe's answer, -1 until
+                                                   // the copy has landed; [1] how often the chunk pool ran dry on this bond
+                                                   // list (written by the device: the pool of the next call is doubled that
+                                                   // many times)
 };
-static thread_local ProbeHint g_hints[4];
-static thread_local int g_hint_next = 0;
+// Per host thread: four remembered bond lists, and ONE pinned block of kHintPairs answer pairs handed out round robin,
+// so that a copy or a device-side store still in flight for a forgotten entry lands in a pair that is not handed out
+// again until kHintPairs - 4 further bond lists have been seen (it could only cost speed, never a result).  The block
+// is released when the thread exits.
+constexpr int kHintPairs = 64;
+struct HintStore {
+    ProbeHint slot[4];
+    int next_slot = 0, next_pair = 0;
+    int32_t* pinned = nullptr;
+    ~HintStore() { if (pinned) { cudaFreeHost(pinned); pinned = nullptr; } }    // (fails harmlessly once the runtime is gone)
+};
+static thread_local HintStore g_hints;
 
 static ProbeHint* hint_find(const void* src, const void* dst, int64_t n_bonds, int64_t n_sites, int shift)
 {
-    for (ProbeHint& h : g_hints)
+    for (ProbeHint& h : g_hints.slot)
         if (h.answer && h.src == src && h.dst == dst && h.n_bonds == n_bonds && h.n_sites == n_sites && h.shift == shift) return &h;
     return nullptr;
 }
 
 // ccl_set_option("probe_cache" | "reset"): what this host thread remembers about bond lists is forgotten (the pinned
-// words are kept for reuse)
+// block is kept for reuse)
 void forget_probe_hints()
 {
-    for (ProbeHint& h : g_hints) { h.src = nullptr; h.dst = nullptr; h.n_bonds = -1; }
+    for (ProbeHint& h : g_hints.slot) { h.src = nullptr; h.dst = nullptr; h.n_bonds = -1; h.answer = nullptr; }
 }
 
 static ProbeHint* hint_new(const void* src, const void* dst, int64_t n_bonds, int64_t n_sites, int shift)
 {
-    ProbeHint& h = g_hints[g_hint_next];
-    g_hint_next = (g_hint_next + 1) % 4;
-    if (h.answer == nullptr && cudaHostAlloc(reinterpret_cast<void**>(&h.answer), 2 * sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) {
-        h.answer = nullptr;
+    HintStore& hs = g_hints;
+    if (hs.pinned == nullptr && cudaHostAlloc(reinterpret_cast<void**>(&hs.pinned), kHintPairs * 2 * sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) {
+        hs.pinned = nullptr;
         cudaGetLastError();
         return nullptr;
     }
+    ProbeHint& h = hs.slot[hs.next_slot];
+    hs.next_slot = (hs.next_slot + 1) % 4;
+    h.answer = hs.pinned + 2 * hs.next_pair;
+    hs.next_pair = (hs.next_pair + 1) % kHintPairs;
     reinterpret_cast<volatile int32_t*>(h.answer)[0] = -1;
     reinterpret_cast<volatile int32_t*>(h.answer)[1] = 0;
     h.src = src; h.dst = dst; h.n_bonds = n_bonds; h.n_sites = n_sites; h.shift = shift;
@@ -511,17 +504,29 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
         if (t.probe_cache) {
             const int shift = bucket_region_shift(n_sites, t);
             hint = hint_find(src, dst, n_bonds, n_sites, shift);
+            if (hint == nullptr) hint = hint_new(src, dst, n_bonds, n_sites, shift);
             if (hint) {
                 const int32_t ans = reinterpret_cast<volatile int32_t*>(hint->answer)[0];
                 if (mode < 0 && (ans == 0 || ans == 1)) mode = ans;
                 pool_doublings = reinterpret_cast<volatile int32_t*>(hint->answer)[1];
-            } else {
-                hint = hint_new(src, dst, n_bonds, n_sites, shift);
-                report_probe = hint != nullptr && mode < 0;
+                // no answer yet (first call, or earlier calls were forced or failed before the copy): ask for it again
+                report_probe = mode < 0;
             }
         }
-        rc = bucketed_begin(n_sites, n_bonds, t, pool_doublings, st, &plan, &bucket_ws);
-        if (rc != CCL_OK) return rc;
+        // The bucketed form is an optimisation: the direct kernels need no workspace.  Nothing is drawn when the remembered
+        // answer is "direct", and when the pool cannot supply the workspace the call goes on with the direct kernels (and
+        // the next call on this bond list asks for a pool half as large again).
+        if (mode != 0) {
+            rc = bucketed_begin(n_sites, n_bonds, t, pool_doublings, st, &plan, &bucket_ws);
+            if (rc != CCL_OK) {
+                cudaGetLastError();
+                if (bucket_ws) { cudaFreeAsync(bucket_ws, st); bucket_ws = nullptr; }
+                if (hint && pool_doublings > 0) reinterpret_cast<volatile int32_t*>(hint->answer)[1] = pool_doublings - 1;
+                plan = BucketPlan();
+                mode = 0;
+                report_probe = false;
+            }
+        }
     }
     auto done = [&](int code) { if (bucket_ws) cudaFreeAsync(bucket_ws, st); return code; };
     const int gate = mode < 0 ? kGateDirectOrOverflow : kGateOverflow;
@@ -531,7 +536,7 @@ static int label_impl(int64_t n_sites, int64_t n_bonds, const int32_t* src, cons
         ProbeJob job;
         if (mode < 0) { job.hdr = plan.hdr; job.n_bonds = n_bonds; job.src = src; job.dst = dst; job.shift = plan.shift; }
         const int64_t site_blocks = (((n_sites + 3) / 4) + kThreads - 1) / kThreads;
-        const int64_t init_blocks = site_blocks < (int64_t)kSMs * 32 ? site_blocks : (int64_t)kSMs * 32;
+        const int64_t init_blocks = site_blocks < (int64_t)sm_count() * 32 ? site_blocks : (int64_t)sm_count() * 32;
         k_init<<<(unsigned)init_blocks, kThreads, 0, st>>>(n_sites, labels, job);                // (+ the probe)
         { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) { set_error("launch of k_init failed: %s", cudaGetErrorString(e)); return done(CCL_CUDA_ERROR); } count_launch(); }
         mark(0, st);
@@ -609,7 +614,7 @@ extern "C" int ccl_validate_bonds(int64_t n_sites, int64_t n_bonds, const int32_
     CCL_CUDA_TRY(cudaMemsetAsync(out_bad, 0, sizeof(int64_t), st));
     if (n_bonds == 0) return CCL_OK;
     int64_t blocks = (n_bonds + kThreads - 1) / kThreads;
-    if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+    if (blocks > (int64_t)sm_count() * 16) blocks = (int64_t)sm_count() * 16;
     k_validate<<<(unsigned)blocks, kThreads, 0, st>>>(n_sites, n_bonds, src, dst,
                                                       reinterpret_cast<unsigned long long*>(out_bad));
     CCL_CHECK_LAUNCH("k_validate");

@@ -86,7 +86,7 @@ extern "C" int ccl_label_nn(int64_t n_sites, int32_t z_max, const int32_t* nn_li
     if (n_sites == 0) return CCL_OK;
     cudaStream_t st = as_stream(stream);
     int64_t blocks = (n_sites + kNnThreads - 1) / kNnThreads;
-    if (blocks > (int64_t)kSMs * 32) blocks = (int64_t)kSMs * 32;
+    if (blocks > (int64_t)sm_count() * 32) blocks = (int64_t)sm_count() * 32;
     k_nn_init<<<(unsigned)blocks, kNnThreads, 0, st>>>(n_sites, z_max, nn_list, labels);          // step (i)
     CCL_CHECK_LAUNCH("k_nn_init");
     if (z_max == 0) return CCL_OK;

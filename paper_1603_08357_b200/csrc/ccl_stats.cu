@@ -96,7 +96,7 @@ extern "C" int ccl_cluster_stats(int64_t n_sites, const int32_t* labels, int32_t
     }
     CCL_CUDA_TRY(cudaMemsetAsync(size_scratch, 0, sizeof(int32_t) * (size_t)n_sites, st));
     int64_t blocks = (n_sites + kStatThreads - 1) / kStatThreads;
-    if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+    if (blocks > (int64_t)sm_count() * 16) blocks = (int64_t)sm_count() * 16;
     k_count_sizes<<<(unsigned)blocks, kStatThreads, 0, st>>>(n_sites, labels, size_scratch);
     CCL_CHECK_LAUNCH("k_count_sizes");
     // best_key lives in out->largest until k_finish_stats unpacks it
@@ -176,7 +176,7 @@ extern "C" int ccl_cluster_stats_static(int64_t n_sites, const int32_t* labels, 
     // the table still holds the sizes of the previous call: the first n_sites counters must start at zero
     CCL_CUDA_TRY(cudaMemsetAsync(sizes, 0, sizeof(int32_t) * (size_t)n_sites, st));
     int64_t blocks = (n_sites + kStatThreads - 1) / kStatThreads;
-    if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+    if (blocks > (int64_t)sm_count() * 16) blocks = (int64_t)sm_count() * 16;
     k_count_sizes<<<(unsigned)blocks, kStatThreads, 0, st>>>(n_sites, labels, sizes);
     CCL_CHECK_LAUNCH("k_count_sizes");
     unsigned long long* best_key = reinterpret_cast<unsigned long long*>(&out->largest);

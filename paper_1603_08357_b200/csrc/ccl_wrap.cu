@@ -159,7 +159,7 @@ extern "C" int ccl_wrap(int64_t n_sites, int64_t n_bonds, const int32_t* src, co
     uint32_t* bits_open = static_cast<uint32_t*>(workspace);
     unsigned long long* node = reinterpret_cast<unsigned long long*>(static_cast<char*>(workspace) + mask_bytes);
     int64_t blocks = ((n_bonds + 31) / 32 + kWrapThreads - 1) / kWrapThreads;
-    if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+    if (blocks > (int64_t)sm_count() * 16) blocks = (int64_t)sm_count() * 16;
     if (n_bonds > 0) {
         k_open_mask<<<(unsigned)blocks, kWrapThreads, 0, st>>>(n_bonds, occupied_bits, wx, wy, bits_open);
         CCL_CHECK_LAUNCH("k_open_mask");
@@ -167,7 +167,7 @@ extern "C" int ccl_wrap(int64_t n_sites, int64_t n_bonds, const int32_t* src, co
     const int rc = ccl_label_bits(n_sites, n_bonds, src, dst, bits_open, labels_open, stream);
     if (rc != CCL_OK || n_bonds == 0) return rc;
     blocks = ((n_bonds + 15) / 16 + kWrapThreads - 1) / kWrapThreads;
-    if (blocks > (int64_t)kSMs * 16) blocks = (int64_t)kSMs * 16;
+    if (blocks > (int64_t)sm_count() * 16) blocks = (int64_t)sm_count() * 16;
     k_wrap_init<<<(unsigned)blocks, kWrapThreads, 0, st>>>(n_bonds, src, dst, occupied_bits, wx, wy, labels_open, node);
     CCL_CHECK_LAUNCH("k_wrap_init");
     k_wrap_union<<<(unsigned)blocks, kWrapThreads, 0, st>>>(n_bonds, src, dst, occupied_bits, wx, wy, labels_open, node, out);

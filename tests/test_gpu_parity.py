@@ -428,6 +428,49 @@ def test_chunk_pool_grows_after_running_dry(ccl):
     ccl.trim_scratch(0)
 
 
+def test_remembered_direct_answer_draws_no_workspace(ccl):
+    """The bucketed form is an optimisation.  Once the probe's answer for a bond list is "direct" and the host remembers
+    it, later calls on that bond list reserve nothing from the pool (include/ccl.h, "What a call draws")."""
+    rng = np.random.default_rng(31)
+    n, m = 300000, 900000
+    src = rng.integers(0, n, size=m).astype(np.int32)
+    dst = np.clip(src + rng.integers(-3, 4, size=m), 0, n - 1).astype(np.int32)      # local in the site numbering
+    s, d = dev(src), dev(dst)
+    want = oracle.label(n, src, dst)
+    ccl.set_option("reset")
+    ccl.set_option("bucket_min_label_bytes", 0)
+    ccl.set_option("region_shift", 13)
+    assert np.array_equal(ccl.label(n, s, d).cpu().numpy(), want)         # first call: both forms behind the probe
+    torch.cuda.synchronize()
+    ccl.trim_scratch(0)
+    assert np.array_equal(ccl.label(n, s, d).cpu().numpy(), want)         # remembered: direct kernels only
+    torch.cuda.synchronize()
+    assert ccl.scratch_bytes() == (0, 0)
+    ccl.set_option("reset")
+
+
+def test_workspace_that_cannot_be_allocated_falls_back_to_the_direct_kernels(ccl):
+    """A pool request the device cannot satisfy (here: room for 2^40 pairs) must not fail the call -- the direct kernels
+    need no workspace -- and must not poison later calls on the same bond list."""
+    rng = np.random.default_rng(32)
+    n, m = 200000, 600000
+    src, dst = graphs.random_graph(rng, n, m)
+    s, d = dev(src), dev(dst)
+    mask = (rng.random(m) < 0.5).astype(np.uint8)
+    want = oracle.label(n, src, dst, mask)
+    for force in (1, -1):
+        ccl.set_tuning(0, 13, force, 1 << 40)
+        for rep in range(2):
+            assert np.array_equal(ccl.label(n, s, d, dev(mask)).cpu().numpy(), want), (force, rep)
+        torch.cuda.synchronize()
+    ccl.set_tuning(0, 13, 1, 0)                                          # an ordinary pool again: the bucketed form runs
+    before = ccl.launch_count()
+    assert np.array_equal(ccl.label(n, s, d, dev(mask)).cpu().numpy(), want)
+    assert ccl.launch_count() - before > 6                                # scatter + one descend per region + ...
+    ccl.set_tuning()
+    ccl.trim_scratch(0)
+
+
 def test_probe_cache_on_and_off(ccl):
     """The host-side memory of the device probe's answer changes which kernels are enqueued, never the labels: repeated
     calls on one bond list (first call: probe undecided, later calls: decided) and the same with the cache off."""
@@ -462,36 +505,6 @@ def test_probe_cache_on_and_off(ccl):
             elif not cache:
                 assert counts[-1] == counts[0]
     ccl.set_option("reset")
-
-
-def test_warp_premerge_option(options):
-    """The pre-merge experiment (profiles/r2_premerge.md) changes which lane sends an atomic, never the labels: one-pass,
-    two-pass and bucketed forms, random graphs, lattices (where lanes really share higher sites), stars, duplicates."""
-    ccl = options
-    rng = np.random.default_rng(4711)
-    for extra in ({"two_pass": 0}, {"two_pass": 1}, {"bucket_min_label_bytes": 0, "region_shift": 11, "force_mode": 1}):
-        ccl.set_option("reset")
-        ccl.set_option("warp_premerge", 1)
-        for k, v in extra.items():
-            ccl.set_option(k, v)
-        for trial in range(10):
-            n = int(rng.integers(2, 80000))
-            m = int(rng.integers(1, 4 * n + 1))
-            src, dst = graphs.random_graph(rng, n, m, self_loops=True)
-            if trial % 2:
-                dst = np.clip(src + rng.integers(-2, 3, size=m), 0, n - 1).astype(np.int32)   # many shared higher sites
-            mask = (rng.random(m) < rng.random()).astype(np.uint8)
-            run_all_forms(ccl, n, src, dst, mask)
-        for name in ["honeycomb_L301", "triangular_L257", "regular4"]:
-            n, src, dst, ps, cfg = _case(name)
-            for p in ps + [1.0]:
-                mask, bits = oracle.gen_occupancy(src.size, p, oracle.seed_for(cfg), realization=11)
-                run_all_forms(ccl, n, src, dst, mask)
-        n = 1 << 15
-        hub = np.full(n - 1, n - 1, dtype=np.int32)
-        assert all_zero(ccl.label(n, dev(hub), dev(np.arange(n - 1, dtype=np.int32))))
-        same = np.full(3000, n - 3, dtype=np.int32)        # 3000 copies of one bond
-        assert ccl.label(n, dev(same), dev(np.full(3000, 7, dtype=np.int32))).cpu().numpy()[n - 3] == 7
 
 
 def test_tuning_argument_checks(ccl):
