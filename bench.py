@@ -318,6 +318,25 @@ class Workload:
         else:
             ccl.label_bits(n, self.src, self.dst, self.masks[k], labels=self.labels)
 
+    def cold_call_ms(self):
+        """Device time of the FIRST call on this bond list: nothing remembered about it (the device-side probe runs and,
+        where the call is eligible for the bucketed form, both forms are enqueued behind it) and the library's memory pool
+        empty (the workspace comes from the driver).  The timed steps below are the warm-sweep steady state."""
+        torch, ccl = self.torch, self.ccl
+        torch.cuda.synchronize()
+        ccl.set_option("probe_cache", 1)                # forgets the remembered bond lists
+        ccl.trim_scratch(0)
+        if self.flush is not None:
+            self.flush.fill_(1)
+        t0 = torch.cuda.Event(enable_timing=True)
+        t1 = torch.cuda.Event(enable_timing=True)
+        wall0 = time.perf_counter()
+        t0.record()
+        self.one_call(0)
+        t1.record()
+        torch.cuda.synchronize()
+        return {"device_ms": t0.elapsed_time(t1), "host_wall_ms": (time.perf_counter() - wall0) * 1e3, "p": self.ps[0]}
+
     def measure(self, K, warmup, barrier, kernel_split=True):
         """W warm-up steps, then K timed steps (one call per p each), CUDA events on the launching stream.  Returns the
         per-call times and the per-step split the library records between its kernels."""
@@ -410,6 +429,7 @@ def run_ours(args):
     torch.cuda.empty_cache()
 
     K = max(1, args.steps)
+    cold = w.cold_call_ms()                 # before anything has warmed up: first call on this bond list
     sampler = ClockSampler(local)
     sampler.start()
     r = w.measure(K, args.warmup, barrier, kernel_split=not args.no_kernel_split)
@@ -446,18 +466,21 @@ def run_ours(args):
             else:
                 ccl.label_bits_host(n, hs, hd, hm[0], hl)
         e2e_step()                                                    # warm-up (memory pool, page tables)
-        e2e_steps = max(1, min(K, 3))
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(e2e_steps):
-            e2e_step()
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        dt = max_over_ranks(dt, world, "cuda")
+        e2e_steps = max(5, min(K, 7))
         h2d = 2 * 4 * m + len(ps) * 4 * ((m + 31) // 32) if sweep else 2 * 4 * m + 4 * ((m + 31) // 32)
         d2h = len(ps) * 4 * n
-        e2e = {"value": world * len(ps) * m * e2e_steps / dt / 1e9, "unit": "Gbonds/s", "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+        dts = []
+        for _ in range(e2e_steps):                                    # every step synchronises: timed one by one
+            barrier()
+            t0 = time.perf_counter()
+            e2e_step()
+            torch.cuda.synchronize()
+            dts.append(max_over_ranks(time.perf_counter() - t0, world, "cuda"))
+        dt = sorted(dts)[len(dts) // 2]                               # the median step
+        e2e = {"value": world * len(ps) * m / dt / 1e9, "unit": "Gbonds/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": e2e_steps, "statistic": "median step",
+               "ms_per_step": {"median": dt * 1e3, "min": min(dts) * 1e3, "max": max(dts) * 1e3},
+               "pcie_gbs_achieved": (h2d + d2h) / dt / 1e9,
                "api": ("ccl_label_sweep_host (pinned host src/dst once + one mask per p in, host labels per p out, synchronous)"
                        if sweep else "ccl_label_bits_host (pinned host src/dst/bits in, host labels out, synchronous)")}
         del hls
@@ -514,6 +537,7 @@ def run_ours(args):
         for name in ("cfg1", "cfg2", "cfg3", "cfg4"):
             wk = Workload(ccl, torch, name, rank)
             torch.cuda.synchronize()
+            cold_k = wk.cold_call_ms()
             rr = wk.measure(5, 3, lambda: torch.cuda.synchronize())
             t = avg(rr["call_ms"])
             configs[name] = {"workload": wk.text, "api": wk.api, "ms_per_call": t, "steps": 5, "warmup": 3,
@@ -522,6 +546,7 @@ def run_ours(args):
                              "roofline_call_frac": wk.call_bytes / (t * 1e-3) / 1e9 / peak,
                              "roofline_call_frac_8TBs": wk.call_bytes / (t * 1e-3) / 1e9 / 8000.0,
                              "gpu_launches_per_call": rr["launches"] / rr["ncalls"], "per_p": wk.per_p(rr, peak),
+                             "cold_first_call": cold_k,
                              "l2": "256 MB buffer rewritten between timed calls" if wk.flush is not None else "inputs larger than L2"}
             del wk
             torch.cuda.empty_cache()
@@ -540,6 +565,13 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "kernel": "k_label_batch (steps i-iv)" if batch > 1 else "step (iii): k_reduce / k_hook + k_join, or k_scatter_tiles + k_descend x regions", "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": stream_bytes, "avg_launch_ms": avg(reduce_ms),
+                         "avg_step_iii_ms": avg(reduce_ms),
+                         "avg_launch_ms_is": "the event-timed duration of step (iii) of one call, which on the bucketed form is "
+                                             "a chain of launches (k_scatter_tiles + one k_descend per region), not one launch; "
+                                             "the largest single kernel is k_descend x regions (profiles/r2_ncu_cfg5.md: 590 of "
+                                             "1224 us per call at p = 0.25)",
+                         "traffic_is": "ncu dram bytes of step (iii) of ONE call at the p named in profiles/traffic.json "
+                                       "(cfg5: p = 0.25 only), while achieved averages the whole p sweep",
                          "share_of_call": avg(reduce_ms) / avg(call_ms)},
             "roofline_call": {"bound": "hbm", "what": "whole ccl_label call, B_min = 8M + mask + 12N (SURVEY 8(d))",
                               "achieved": call_ach, "peak": peak, "unit": "GB/s", "frac": call_ach / peak,
@@ -551,7 +583,9 @@ def run_ours(args):
                 "k_flatten (step iv)": {"algorithmic_bytes": 8 * n, "avg_ms": avg(flat_ms),
                                         "frac": 8 * n / (avg(flat_ms) * 1e-3) / 1e9 / peak}},
             "per_p": per_p, "kernel_ms": {"k_init": avg(init_ms), "k_reduce": avg(reduce_ms), "k_flatten": avg(flat_ms)},
-            "configs": configs,
+            "configs": configs, "cold_first_call": cold,
+            "timed_state": "warm sweep: the probe's answer for the bond list is remembered and the memory pool is reserved "
+                           "(>= 3 warm-up sweeps on the same src/dst); cold_first_call is the first call without either",
             "statistics": statistics, "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
         }
         print(json.dumps(line), flush=True)

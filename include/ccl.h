@@ -241,6 +241,11 @@ int ccl_scratch_bytes(int64_t* reserved, int64_t* in_use);
  *   "flatten_window_bytes"    step (iv) behind the bucketed form gathers from one window of label[] of this many bytes
  *                             at a time (default 64 MiB, what stays resident in L2);
  *   "flatten_window_min_bytes" ... for label arrays of at least this many bytes (default 96 MiB; 0 = always; < 0 = never)
+ *   "l2_persist"              1 = the k_descend and windowed k_flatten launches of the bucketed form carry a per-launch
+ *                             access-policy window (persisting) over the slice of labels[] they work on.  Default 0:
+ *                             measured slower on B200 (profiles/r3_l2_window.md).  SIDE EFFECT when on: the first such
+ *                             call raises the device-wide limit cudaLimitPersistingL2CacheSize to the device's maximum
+ *                             (79 MiB of the 126.5 MiB L2 on B200), which stays in force for the whole process
  *   "reset"                   all defaults (value ignored); also forgets the remembered bond lists
  * Unknown names -> CCL_INVALID_ARG. */
 int ccl_set_option(const char* name, int64_t value);

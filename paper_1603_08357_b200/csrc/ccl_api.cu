@@ -41,6 +41,35 @@ int sm_count()
     return n;
 }
 
+// Persisting-L2 set-up, once per device: the limit is raised to the device's maximum the first time a launch asks
+// for an access-policy window (ccl_set_option "l2_persist").
+struct L2Persist { bool ready = false; size_t persist = 0, max_window = 0; };
+static std::mutex g_l2_mutex;
+static L2Persist g_l2[64];
+
+static L2Persist l2_state()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return L2Persist(); }
+    std::lock_guard<std::mutex> lock(g_l2_mutex);
+    L2Persist& s = g_l2[dev];
+    if (!s.ready) {
+        int max_persist = 0, max_window = 0;
+        cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
+        cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
+        if (max_persist > 0 && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)max_persist) == cudaSuccess) {
+            size_t got = 0;
+            if (cudaDeviceGetLimit(&got, cudaLimitPersistingL2CacheSize) == cudaSuccess) s.persist = got;
+        }
+        cudaGetLastError();
+        s.max_window = max_window > 0 ? (size_t)max_window : 0;
+        s.ready = true;
+    }
+    return s;
+}
+size_t l2_persist_bytes() { return l2_state().persist; }
+size_t l2_max_window_bytes() { return l2_state().max_window; }
+
 static std::mutex g_pool_mutex;
 static cudaMemPool_t g_pools[64] = {};
 
@@ -117,6 +146,7 @@ extern "C" int ccl_set_option(const char* name, int64_t value)
         return CCL_OK;
     }
     if (!strcmp(name, "flatten_window_min_bytes")) { t.flatten_window_min_bytes = value; return CCL_OK; }
+    if (!strcmp(name, "l2_persist")) { t.l2_persist = value != 0; return CCL_OK; }
     ccl::set_error("invalid argument: unknown option '%s'", name);
     return CCL_INVALID_ARG;
 }

@@ -405,6 +405,7 @@ int bucketed_begin(int64_t n_sites, int64_t n_bonds, const Tuning& t, int pool_d
     plan->cshift = cshift;
     plan->n_regions = n_regions;
     plan->scatter_tiles = t.scatter_tiles;
+    plan->l2_persist = t.l2_persist;
     CCL_CUDA_TRY(cudaMemsetAsync(ws, 0, hdr_bytes + table_bytes, st));
     return CCL_OK;
 }
@@ -463,7 +464,13 @@ int bucketed_launch(const BucketPlan& plan, int64_t n_sites, int64_t n_bonds, co
             init_hi = (int64_t)r << shift;
             if (init_hi > n_sites) init_hi = n_sites;
         }
-        CCL_CUDA_TRY(launch_pdl(k_descend, (unsigned)grids.descend, (unsigned)kBThreads, st, r, bk, gated, init_lo, init_hi, labels));
+        L2Window win;                                                  // region r's labels: every atomic of this launch lands there
+        if (plan.l2_persist) {
+            const int64_t lo = (int64_t)r << shift, hi = ((int64_t)(r + 1) << shift) < n_sites ? ((int64_t)(r + 1) << shift) : n_sites;
+            win.base = labels + lo;
+            win.bytes = (size_t)(hi - lo) * sizeof(int32_t);
+        }
+        CCL_CUDA_TRY(launch_pdl_window(k_descend, (unsigned)grids.descend, (unsigned)kBThreads, 0, st, win, r, bk, gated, init_lo, init_hi, labels));
         count_launch();
     }
     return CCL_OK;

@@ -90,6 +90,50 @@ inline cudaError_t launch_pdl_smem(void (*kernel)(Params...), unsigned grid, uns
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
 }
 
+// ---- L2 residency: a per-launch access-policy window ---------------------------------------------------------
+// The bucketed form works on one slice of label[] at a time (a region in k_descend, a gather window in k_flatten).
+// With ccl_set_option("l2_persist", 1) those launches carry cudaLaunchAttributeAccessPolicyWindow over their slice
+// (hitProp = persisting), so that the streams passing through L2 in the same launch (pair chunks, the sites above
+// the window) do not push the slice out.  l2_persist_bytes() sets the device-wide limit
+// cudaLimitPersistingL2CacheSize to the device's maximum on first use (a side effect on the whole device, documented
+// in include/ccl.h) and returns it; 0 = not available.
+struct L2Window {
+    const void* base = nullptr;
+    size_t bytes = 0;                              // 0: no window
+};
+size_t l2_persist_bytes();
+size_t l2_max_window_bytes();
+
+template <typename... Params, typename... Args>
+inline cudaError_t launch_pdl_window(void (*kernel)(Params...), unsigned grid, unsigned block, size_t smem, cudaStream_t st,
+                                     L2Window win, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[2];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const size_t persist = win.bytes ? l2_persist_bytes() : 0;
+    if (persist > 0) {
+        size_t bytes = win.bytes;
+        const size_t max_window = l2_max_window_bytes();
+        if (max_window > 0 && bytes > max_window) bytes = max_window;
+        attr[1].id = cudaLaunchAttributeAccessPolicyWindow;
+        attr[1].val.accessPolicyWindow.base_ptr = const_cast<void*>(win.base);
+        attr[1].val.accessPolicyWindow.num_bytes = bytes;
+        attr[1].val.accessPolicyWindow.hitRatio = bytes <= persist ? 1.0f : (float)((double)persist / (double)bytes);
+        attr[1].val.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+        attr[1].val.accessPolicyWindow.missProp = cudaAccessPropertyNormal;
+        cfg.numAttrs = 2;
+    }
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
+}
+
 // ---- region-bucketed label reduction (ccl_bucket.cu) -----------------------------------------------------
 constexpr int kMaxRegions = 32;
 constexpr int kMinChunkShift = 11, kMaxChunkShift = 21;   // a bucket is a sequence of chunks of 2^11 .. 2^21 pairs
@@ -115,6 +159,7 @@ struct Tuning {                                    // ccl_set_option(); one set 
     int32_t probe_cache = 1;                       // remember the probe's answer per bond list (host side, hint only)
     int64_t flatten_window_bytes = 64ll << 20;     // step (iv) gathers from one L2-resident window of label[] at a time
     int64_t flatten_window_min_bytes = 96ll << 20; // ... for label arrays of at least this size (0: always; < 0: never)
+    int32_t l2_persist = 0;                        // 1: k_descend / windowed k_flatten launches carry an access-policy window
 };
 Tuning& tuning();
 
@@ -139,6 +184,7 @@ struct BucketPlan {
     int shift = 0, n_regions = 0;
     int cshift = kMinChunkShift;                   // chunk = 2^cshift pairs
     int scatter_tiles = 1;
+    int l2_persist = 0;
     int lazy_init = 0;                             // 1: label[] of region r is written by the kernel that runs before k_descend(r)
     int gated = 0;                                 // 1: the kernels return at once unless hdr->mode == 1 (probe undecided on the host)
 };

@@ -359,10 +359,12 @@ static int launch_reduce(int64_t n_bonds, const int32_t* src, const int32_t* dst
 }
 
 static int launch_flatten(int64_t n_sites, int32_t* labels, int64_t lo, int64_t hi, const BucketHeader* hdr, int gate,
-                          cudaStream_t st)
+                          cudaStream_t st, bool persist_window = false)
 {
     const int64_t blocks = (((n_sites - lo + 3) / 4) + kThreads - 1) / kThreads;
-    const cudaError_t e = launch_pdl(k_flatten, (unsigned)blocks, (unsigned)kThreads, st, n_sites, labels, lo, hi, hdr, gate);
+    L2Window win;                                          // the gather window [lo, hi) of a windowed step (iv)
+    if (persist_window) { win.base = labels + lo; win.bytes = (size_t)(hi - lo) * sizeof(int32_t); }
+    const cudaError_t e = launch_pdl_window(k_flatten, (unsigned)blocks, (unsigned)kThreads, 0, st, win, n_sites, labels, lo, hi, hdr, gate);
     if (e != cudaSuccess) { set_error("launch of k_flatten failed: %s", cudaGetErrorString(e)); return CCL_CUDA_ERROR; }
     count_launch();
     return CCL_OK;
@@ -399,7 +401,8 @@ static int flatten_all(int64_t n_sites, int32_t* labels, bool windowed, const Tu
         w &= ~(int64_t)3;
     }
     for (int64_t lo = 0; lo < n_sites; lo += w) {
-        const int rc = launch_flatten(n_sites, labels, lo, lo + w < n_sites ? lo + w : n_sites, nullptr, kGateNone, st);
+        const int rc = launch_flatten(n_sites, labels, lo, lo + w < n_sites ? lo + w : n_sites, nullptr, kGateNone, st,
+                                      t.l2_persist && w < n_sites);
         if (rc != CCL_OK) return rc;
     }
     return CCL_OK;

@@ -471,6 +471,27 @@ def test_workspace_that_cannot_be_allocated_falls_back_to_the_direct_kernels(ccl
     ccl.trim_scratch(0)
 
 
+def test_l2_persist_option_changes_no_label(ccl):
+    """ccl_set_option("l2_persist", 1) attaches an access-policy window to the k_descend / windowed k_flatten launches:
+    a cache hint, so the labels are the oracle's either way (bucketed form forced on small graphs, several regions and
+    several flatten windows)."""
+    rng = np.random.default_rng(77)
+    n, m = 150000, 400000
+    src, dst = graphs.random_graph(rng, n, m, self_loops=True)
+    mask = (rng.random(m) < 0.55).astype(np.uint8)
+    want = oracle.label(n, src, dst, mask)
+    s, d, mk = dev(src), dev(dst), dev(mask)
+    for on in (1, 0):
+        ccl.set_tuning(0, 14, 1, 0)
+        ccl.set_option("flatten_window_min_bytes", 0)
+        ccl.set_option("flatten_window_bytes", 1 << 17)
+        ccl.set_option("l2_persist", on)
+        for rep in range(2):
+            assert np.array_equal(ccl.label(n, s, d, mk).cpu().numpy(), want), (on, rep)
+    ccl.set_tuning()
+    ccl.trim_scratch(0)
+
+
 def test_probe_cache_on_and_off(ccl):
     """The host-side memory of the device probe's answer changes which kernels are enqueued, never the labels: repeated
     calls on one bond list (first call: probe undecided, later calls: decided) and the same with the cache off."""
