@@ -108,15 +108,17 @@ __device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_
 
 // One pass over the bond stream.  About a quarter of the occupied bonds survive the first touch and need root
 // walks, which are long chains of dependent L2 loads; left where they arise they would keep a quarter of the lanes
-// busy for four rounds.  So every warp packs its survivors into a shared-memory queue and then works through the
-// queue with all lanes.
+// busy for four rounds.  So every warp packs its survivors into a shared-memory queue and works through the queue
+// 32 pairs at a time, every lane busy; fewer than 32 pairs stay queued for the next iteration (the order in which
+// bonds are joined is free), at most 31 + 128 of them.
+constexpr int kQueueSlots = 160;
 template <int MASK, bool VEC>
 __global__ void __launch_bounds__(kThreads)
 k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
          const void* __restrict__ occ, int32_t* label, const BucketHeader* hdr, int gate,
          int32_t* notify, int32_t notify_value)
 {
-    __shared__ int2 queue[kThreads / 32][128];
+    __shared__ int2 queue[kThreads / 32][kQueueSlots];
     pdl_wait();
     if (!gate_open(hdr, gate)) return;                     // the bucketed form (ccl_bucket.cu) did step (iii)
     // Running as the safety net of the bucketed form (its chunk pool ran dry): tell the host, through mapped pinned
@@ -129,6 +131,7 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
     const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
+    int qn = 0;                                            // pairs waiting in this warp's queue (the same in every lane)
     for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
         int32_t pa[4], pb[4];
         const int n = reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol, pa, pb);
@@ -140,16 +143,22 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
         }
         const int total = __shfl_sync(0xffffffffu, incl, 31);
         if (total == 0) continue;
-        const int off = incl - n;
+        const int off = qn + incl - n;
 #pragma unroll
         for (int q = 0; q < 4; ++q)
             if (q < n) queue[warp][off + q] = make_int2(pa[q], pb[q]);
+        qn += total;
         __syncwarp();
-        for (int j = lane; j < total; j += 32) {
-            const int2 pr = queue[warp][j];
+        while (qn >= 32) {                                 // whole rounds only: every lane has a pair to walk
+            qn -= 32;
+            const int2 pr = queue[warp][qn + lane];
             algorithm1(label, pr.x, pr.y);
         }
         __syncwarp();
+    }
+    if (lane < qn) {                                       // what is left at the end of the warp's share of the bonds
+        const int2 pr = queue[warp][lane];
+        algorithm1(label, pr.x, pr.y);
     }
 }
 
@@ -185,13 +194,14 @@ __global__ void __launch_bounds__(kThreads)
 k_join(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restrict__ dst, const void* __restrict__ occ,
        int vec, int32_t* label, const BucketHeader* hdr, int gate)
 {
-    __shared__ int2 queue[kThreads / 32][128];
+    __shared__ int2 queue[kThreads / 32][kQueueSlots];
     pdl_wait();
     if (!gate_open(hdr, gate)) return;
     const uint64_t pol = evict_first_policy();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
     const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
+    int qn = 0;                                            // as in k_reduce: whole rounds of 32 pairs, the rest waits
     for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
         const Bonds4 c = load_bonds4<MASK>(n_bonds, b0, src, dst, occ, vec, pol);
         // labels of both ends, all eight loads in flight; after the flatten they are roots unless k_join moved them
@@ -213,16 +223,22 @@ k_join(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restri
         }
         const int total = __shfl_sync(0xffffffffu, incl, 31);
         if (total == 0) continue;
-        int off = incl - n;
+        int off = qn + incl - n;
 #pragma unroll
         for (int k = 0; k < 4; ++k)
             if (la[k] != lb[k]) queue[warp][off++] = make_int2(la[k], lb[k]);     // joining the two labels joins the two sites
+        qn += total;
         __syncwarp();
-        for (int j = lane; j < total; j += 32) {
-            const int2 pr = queue[warp][j];
+        while (qn >= 32) {
+            qn -= 32;
+            const int2 pr = queue[warp][qn + lane];
             algorithm1(label, pr.x, pr.y);
         }
         __syncwarp();
+    }
+    if (lane < qn) {
+        const int2 pr = queue[warp][lane];
+        algorithm1(label, pr.x, pr.y);
     }
 }
 
