@@ -12,16 +12,13 @@ struct Bonds4 {
     uint32_t m;
 };
 
+// Loaded in two halves, so that a kernel can fetch the occupancy bits of its NEXT four bonds while it works on the
+// current ones: the mask word and the endpoints are two dependent trips to HBM otherwise (the endpoints of a group
+// without an occupied bond are never fetched).
 template <int MASK>
-__device__ __forceinline__ Bonds4 load_bonds4(int64_t n_bonds, int64_t b0, const int32_t* __restrict__ src,
-                                              const int32_t* __restrict__ dst, const void* __restrict__ occ, int vec,
-                                              uint64_t pol)
+__device__ __forceinline__ uint32_t load_mask4(int64_t n_bonds, int64_t b0, const void* __restrict__ occ, int vec, uint64_t pol)
 {
-    Bonds4 r;
-    r.m = 0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) { r.u[k] = 0; r.v[k] = 0; }
-    if (b0 >= n_bonds) return r;
+    if (b0 >= n_bonds) return 0;
     const int cnt = (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
     uint32_t m = 0xFu;
     if (MASK == 2) {
@@ -37,9 +34,18 @@ __device__ __forceinline__ Bonds4 load_bonds4(int64_t n_bonds, int64_t b0, const
             for (int k = 0; k < cnt; ++k) m |= (uint32_t)(ld_stream_u8(o + k, pol) != 0) << k;
         }
     }
-    m &= (1u << cnt) - 1u;
+    return m & ((1u << cnt) - 1u);
+}
+
+__device__ __forceinline__ Bonds4 load_ends4(int64_t n_bonds, int64_t b0, uint32_t m, const int32_t* __restrict__ src,
+                                             const int32_t* __restrict__ dst, int vec, uint64_t pol)
+{
+    Bonds4 r;
     r.m = m;
-    if (m == 0) return r;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { r.u[k] = 0; r.v[k] = 0; }
+    if (m == 0) return r;                                  // (also: b0 >= n_bonds)
+    const int cnt = (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
     if (vec && cnt == 4) {
         const int4 s = ld_stream_v4(src + b0, pol), d = ld_stream_v4(dst + b0, pol);
         r.u[0] = s.x; r.u[1] = s.y; r.u[2] = s.z; r.u[3] = s.w;

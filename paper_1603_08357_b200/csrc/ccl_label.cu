@@ -39,57 +39,21 @@ __device__ __forceinline__ bool gate_open(const BucketHeader* hdr, int kind)
 // ---------------------------------------------------------------------------------------------- step (iii)
 // MASK: 0 = every bond occupied, 1 = uint8 per bond, 2 = packed bits.  VEC: src/dst 16-byte aligned (and the
 // uint8 mask 4-byte aligned), so a thread fetches its 4 bonds with two 128-bit loads.
-template <int MASK, bool VEC>
-__device__ __forceinline__ int reduce4(int64_t n_bonds, int64_t b0, const int32_t* __restrict__ src,
-                                       const int32_t* __restrict__ dst, const void* __restrict__ occ,
-                                       int32_t* label, uint64_t pol, int32_t (&pa)[4], int32_t (&pb)[4])
+//
+// First touch of a thread's (up to) 4 bonds: Algorithm 1's atomicMin applied straight to the bond's own endpoints, all
+// four in flight at once.  If the higher site was still a root this IS the link (the paper's step (i) hook,
+// PAPER.md:113, done as the first wave of step (iii)); otherwise the returned value tells which pair is left to join.
+// Returns how many pairs are left; they are stored in pa[]/pb[] front-packed.
+__device__ __forceinline__ int first_touch4(const Bonds4& c, int32_t* label, int32_t (&pa)[4], int32_t (&pb)[4])
 {
-    // Loads this thread's (up to) 4 bonds, does the first-touch atomics, and returns how many pairs are left to join;
-    // they are stored in pa[]/pb[] front-packed.
-    if (b0 >= n_bonds) return 0;
-    const int cnt = (n_bonds - b0 >= 4) ? 4 : (int)(n_bonds - b0);
-
-    // occupancy of this thread's 4 bonds -> low 4 bits of m
-    uint32_t m = 0xFu;
-    if (MASK == 2) {
-        m = (ld_stream_u32(static_cast<const uint32_t*>(occ) + (b0 >> 5), pol) >> (b0 & 31)) & 0xFu;   // b0 % 4 == 0
-    } else if (MASK == 1) {
-        const uint8_t* o = static_cast<const uint8_t*>(occ) + b0;
-        if (VEC && cnt == 4) {
-            const uint32_t w = ld_stream_u32(reinterpret_cast<const uint32_t*>(o), pol);
-            m = ((w & 0xFFu) != 0) | (((w & 0xFF00u) != 0) << 1) | (((w & 0xFF0000u) != 0) << 2) |
-                (((w & 0xFF000000u) != 0) << 3);
-        } else {
-            m = 0;
-            for (int k = 0; k < cnt; ++k) m |= (uint32_t)(ld_stream_u8(o + k, pol) != 0) << k;
-        }
-    }
-    m &= (1u << cnt) - 1u;
-    if (m == 0) return 0;
-
-    int32_t u[4] = {0, 0, 0, 0}, v[4] = {0, 0, 0, 0};
-    if (VEC && cnt == 4) {
-        const int4 s = ld_stream_v4(src + b0, pol), d = ld_stream_v4(dst + b0, pol);
-        u[0] = s.x; u[1] = s.y; u[2] = s.z; u[3] = s.w;
-        v[0] = d.x; v[1] = d.y; v[2] = d.z; v[3] = d.w;
-    } else {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            u[k] = (k < cnt) ? ld_stream_s32(src + b0 + k, pol) : 0;
-            v[k] = (k < cnt) ? ld_stream_s32(dst + b0 + k, pol) : 0;
-        }
-    }
-
-    // First touch: Algorithm 1's atomicMin applied straight to the bond's own endpoints, all four in flight at
-    // once.  If the higher site was still a root this IS the link (the paper's step (i) hook, done
-    // as the first wave of step (iii)); otherwise the returned value tells which pair is left to join.
+    if (c.m == 0) return 0;
     int32_t lo[4], old[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        lo[k] = min(u[k], v[k]);
-        const int32_t hi = max(u[k], v[k]);
+        lo[k] = min(c.u[k], c.v[k]);
+        const int32_t hi = max(c.u[k], c.v[k]);
         old[k] = lo[k];                                    // "nothing left to do"
-        const bool need = ((m >> k) & 1u) && hi != lo[k];
+        const bool need = ((c.m >> k) & 1u) && hi != lo[k];
         if (need) {
             const int32_t o = atomicMin(label + hi, lo[k]);
             old[k] = (o == hi) ? lo[k] : o;
@@ -132,9 +96,14 @@ k_reduce(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __rest
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
     const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
     int qn = 0;                                            // pairs waiting in this warp's queue (the same in every lane)
-    for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
+    int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
+    uint32_t m_next = load_mask4<MASK>(n_bonds, b0, occ, VEC, pol);
+    for (; b0 < n_round; b0 += stride) {
+        // this iteration's endpoints and the next iteration's occupancy bits travel together
+        const Bonds4 c = load_ends4(n_bonds, b0, m_next, src, dst, VEC, pol);
+        m_next = load_mask4<MASK>(n_bonds, b0 + stride, occ, VEC, pol);
         int32_t pa[4], pb[4];
-        const int n = reduce4<MASK, VEC>(n_bonds, b0, src, dst, occ, label, pol, pa, pb);
+        const int n = first_touch4(c, label, pa, pb);
         int incl = n;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -178,8 +147,11 @@ k_hook(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restri
     const uint64_t pol = evict_first_policy();
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
     const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
-    for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
-        const Bonds4 c = load_bonds4<MASK>(n_bonds, b0, src, dst, occ, vec, pol);
+    int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
+    uint32_t m_next = load_mask4<MASK>(n_bonds, b0, occ, vec, pol);
+    for (; b0 < n_round; b0 += stride) {
+        const Bonds4 c = load_ends4(n_bonds, b0, m_next, src, dst, vec, pol);
+        m_next = load_mask4<MASK>(n_bonds, b0 + stride, occ, vec, pol);
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const bool need = ((c.m >> k) & 1u) && c.u[k] != c.v[k];
@@ -202,8 +174,11 @@ k_join(int64_t n_bonds, const int32_t* __restrict__ src, const int32_t* __restri
     const int64_t stride = (int64_t)gridDim.x * kThreads * 4;
     const int64_t n_round = ((n_bonds + 127) / 128) * 128;                 // whole warps take part in every round
     int qn = 0;                                            // as in k_reduce: whole rounds of 32 pairs, the rest waits
-    for (int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; b0 < n_round; b0 += stride) {
-        const Bonds4 c = load_bonds4<MASK>(n_bonds, b0, src, dst, occ, vec, pol);
+    int64_t b0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
+    uint32_t m_next = load_mask4<MASK>(n_bonds, b0, occ, vec, pol);
+    for (; b0 < n_round; b0 += stride) {
+        const Bonds4 c = load_ends4(n_bonds, b0, m_next, src, dst, vec, pol);
+        m_next = load_mask4<MASK>(n_bonds, b0 + stride, occ, vec, pol);
         // labels of both ends, all eight loads in flight; after the flatten they are roots unless k_join moved them
         int32_t la[4], lb[4];
 #pragma unroll
