@@ -38,10 +38,11 @@ k_nn_init(int64_t n_sites, int z_max, const int32_t* __restrict__ nn, int32_t* _
 __global__ void __launch_bounds__(kNnThreads)
 k_nn_reduce(int64_t n_sites, int z_max, const int32_t* __restrict__ nn, int32_t* label)
 {
-    __shared__ int2 queue[kNnThreads / 32][32];
+    __shared__ int2 queue[kNnThreads / 32][64];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * kNnThreads;
     const int64_t n_round = ((n_sites + 31) / 32) * 32;                    // whole warps take part in every round
+    int qn = 0;                                                            // pairs waiting in the warp's queue (< 32 between looks)
     for (int64_t i = (int64_t)blockIdx.x * kNnThreads + threadIdx.x; i < n_round; i += stride) {
         const bool live = i < n_sites;
         for (int k = 0; k < z_max; ++k) {
@@ -56,17 +57,24 @@ k_nn_reduce(int64_t n_sites, int z_max, const int32_t* __restrict__ nn, int32_t*
                 lb = ld_label(label + j);
                 need = la != lb;
             }
-            // the pairs that are not visibly joined are packed and worked off by all lanes (walks diverge badly otherwise)
+            // the pairs that are not visibly joined are packed and worked off 32 at a time, every lane busy (walks diverge
+            // badly otherwise); fewer than 32 wait for the next look -- the order of the joins is free
             const unsigned m = __ballot_sync(0xffffffffu, need);
             if (m == 0) continue;
-            if (need) queue[warp][__popc(m & ((1u << lane) - 1u))] = make_int2(la, lb);
+            if (need) queue[warp][qn + __popc(m & ((1u << lane) - 1u))] = make_int2(la, lb);
+            qn += __popc(m);
             __syncwarp();
-            if (lane < __popc(m)) {
-                const int2 pr = queue[warp][lane];
+            if (qn >= 32) {
+                qn -= 32;
+                const int2 pr = queue[warp][qn + lane];
                 algorithm1(label, pr.x, pr.y);
             }
             __syncwarp();
         }
+    }
+    if (lane < qn) {
+        const int2 pr = queue[warp][lane];
+        algorithm1(label, pr.x, pr.y);
     }
 }
 
