@@ -69,6 +69,21 @@ def test_no_cpu_fallback_without_a_device():
         binding.label(4, torch.zeros(2, dtype=torch.int32), torch.zeros(2, dtype=torch.int32))
 
 
+def test_every_option_is_documented_in_the_header():
+    """Every name ccl_set_option accepts is described in include/ccl.h, and the header names no option that is gone."""
+    with open(os.path.join(ROOT, "paper_1603_08357_b200", "csrc", "ccl_api.cu")) as f:
+        accepted = set(re.findall(r'strcmp\(name, "([a-z0-9_]+)"\)', f.read()))
+    with open(os.path.join(ROOT, "include", "ccl.h")) as f:
+        text = f.read()
+    block = text[text.index("ccl_set_option(name, value)"):text.index("int ccl_set_option(")]
+    documented = set(re.findall(r'^ \*   "([a-z0-9_]+)"', block, flags=re.M))
+    assert accepted and accepted == documented, (sorted(accepted - documented), sorted(documented - accepted))
+    from paper_1603_08357_b200 import binding
+    for name in sorted(accepted):
+        assert binding.lib.ccl_set_option(name.encode(), -1 if name != "region_shift" else 20) == 0, name
+    assert binding.lib.ccl_set_option(b"reset", 0) == 0
+
+
 def test_product_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_1603_08357_b200")
     for dirpath, _, files in os.walk(pkg):
