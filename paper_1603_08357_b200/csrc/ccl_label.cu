@@ -367,7 +367,9 @@ static int launch_two_pass(int64_t n_sites, int64_t n_bonds, const int32_t* src,
 {
     const int64_t groups = (n_bonds + 3) / 4;
     int64_t blocks = (groups + kThreads - 1) / kThreads;
-    if (blocks > (int64_t)sm_count() * 8 * 4) blocks = (int64_t)sm_count() * 8 * 4;
+    // one resident wave, grid-stride (measured on cfg2: 1 / 4 / 8 / 16 waves 0.458 / 0.467 / 0.474 / 0.496 ms; the one-pass
+    // kernel above is the other way round on the honeycomb lattice: 0.777 / 0.683 / 0.683 / 0.704 ms)
+    if (blocks > (int64_t)sm_count() * 8) blocks = (int64_t)sm_count() * 8;
     uintptr_t a = reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst);
     int vec = (a & 15) == 0;
     if (MASK == 1) vec = vec && (reinterpret_cast<uintptr_t>(occ) & 3) == 0;
