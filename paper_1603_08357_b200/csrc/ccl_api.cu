@@ -107,7 +107,7 @@ int scratch_alloc(void** ptr, size_t bytes, cudaStream_t st)
 }  // namespace ccl
 
 extern "C" const char* ccl_last_error(void) { return ccl::g_error; }
-extern "C" int ccl_version(void) { return 300; }      // 0.3.0: chunked bucket pool, windowed step (iv), scratch trim, per-thread options
+extern "C" int ccl_version(void) { return 400; }      // 0.4.0: ccl_cluster_stats_static, whole-round survivor walks, per-device set-up, l2_persist option
 extern "C" int64_t ccl_launch_count(void) { return ccl::g_launches; }
 
 extern "C" int ccl_set_option(const char* name, int64_t value)
